@@ -1,0 +1,220 @@
+"""Pins for the oracle's whole-ray integration and shadow statistics (-m "not gpu")."""
+import numpy as np
+import pytest
+
+import closed_forms as cf
+import golden_values
+import oracle as o
+
+GOLD = golden_values.load()
+
+
+def _grid(W, nx, ny):
+    al = -W + (np.arange(nx) + 0.5) * 2 * W / nx
+    be = -W + (np.arange(ny) + 0.5) * 2 * W / ny
+    A, B = np.meshgrid(al, be)          # beta slow
+    return A.ravel(), B.ravel()
+
+
+def test_schwarzschild_critical_impact_parameter_sqrt27():
+    # BASELINE config C1: a = 0, i = 60 deg, 64 x 64 over +-10 M; captured <=> sqrt(alpha^2 + beta^2) < sqrt(27)
+    res = o.trace(0.0, 1000.0, 60.0, 10.0, 64, 64, rule=o.STEP_EQ2, threads=4)
+    al, be = _grid(10.0, 64, 64)
+    b = np.hypot(al, be)
+    cap = res["status"] == o.CAPTURED
+    assert np.all(np.isin(res["status"], (o.CAPTURED, o.ESCAPED)))
+    bad = cap != (b < np.sqrt(27.0))
+    assert np.all(np.abs(b[bad] / np.sqrt(27.0) - 1) < 0.01)
+    assert bad.sum() == 0       # measured: the paper's eq. (2) rule classifies every C1 pixel correctly
+
+
+def test_rel_rule_misclassifies_as_design_md_states():
+    # DESIGN.md reading R5: the configs' literal rule dlambda = -h r, tested after full steps only,
+    # jumps the band [r_h, 1.01 r_h] and misclassifies pixels deep inside the shadow.  This test
+    # documents the failure (it is the reason the physical checks run with eq. (2)).
+    res = o.trace(0.0, 1000.0, 60.0, 10.0, 64, 64, rule=o.STEP_REL, threads=4)
+    al, be = _grid(10.0, 64, 64)
+    b = np.hypot(al, be)
+    bad = (res["status"] == o.CAPTURED) != (b < np.sqrt(27.0))
+    assert 20 < bad.sum() < 400
+    assert np.any(b[bad] < 0.9 * np.sqrt(27.0))
+
+
+@pytest.mark.parametrize("a,inc,W", [(0.9, 60.0, 10.0), (0.99, 90.0, 12.0), (0.7, 45.0, 15.0), (0.5, 5.0, 10.0)])
+def test_kerr_capture_matches_radial_potential_classifier(a, inc, W):
+    # exact per-ray classifier independent of the integrator: (xi, eta) of the initial state and
+    # the roots of the radial quartic
+    n = 48
+    res = o.trace(a, 1000.0, inc, W, n, n, rule=o.STEP_EQ2, threads=4)
+    exact = np.zeros(n * n, dtype=bool)
+    for p, y0 in enumerate(res["y0"]):
+        E, L, Q, _ = o.invariants(a, y0)
+        exact[p] = cf.captured_exact(a, L / E, Q / E ** 2)
+    cap = res["status"] == o.CAPTURED
+    assert np.all(np.isin(res["status"], (o.CAPTURED, o.ESCAPED)))
+    al, be = _grid(W, n, n)
+    rho_c = cf.bardeen_rho(a, inc, np.arctan2(be, al))
+    bad = cap != exact
+    assert np.all(np.abs(np.hypot(al, be)[bad] / rho_c[bad] - 1) < 0.01)
+    assert bad.mean() <= 1e-3
+    # and the exact classifier itself agrees with the Bardeen curve away from the edge
+    far = np.abs(np.hypot(al, be) / rho_c - 1) > 0.01
+    assert np.array_equal(exact[far], (np.hypot(al, be) < rho_c)[far])
+
+
+def test_schwarzschild_deflection_matches_orbit_integral():
+    # a = 0, observer in the equatorial plane, beta = 0: the ray stays at theta = pi/2 and its total
+    # sweep in phi between the radii actually used is the textbook orbit integral
+    for alpha in (5.4, 6.0, 8.0, 14.0):
+        y0 = o.init_ray(0.0, 1000.0, 90.0, alpha, 0.0)
+        rh = 2.0
+        y, st, n = o.integrate(0.0, y0, 1 / 32, 1.01 * rh, 1010.0, o.STEP_EQ2, 20000)
+        assert st == o.ESCAPED
+        assert abs(y[2] - np.pi / 2) < 1e-12
+        E, L, _, _ = o.invariants(0.0, y0)
+        b = abs(L / E)
+        exact = cf.schwarzschild_dphi(b, y0[1], y[1])
+        # traced backwards: phi decreases for L < 0 ... compare magnitudes of the sweep
+        got = abs(y[3] - y0[3])
+        assert abs(got - exact) < 2e-5 * exact, (alpha, got, exact)
+        assert exact > np.pi            # light bending: more than a straight line's pi
+
+
+def test_reflection_symmetries():
+    # equatorial reflection: (i, beta) -> (180 - i, -beta) maps theta -> pi - theta
+    a = 0.9
+    for al, be in [(4.0, 3.0), (-6.0, 2.0), (2.0, -1.0)]:
+        y1, s1, n1 = o.integrate(a, o.init_ray(a, 1000.0, 60.0, al, be), 1 / 32, 1.01 * o.horizon(a), 1010.0, o.STEP_EQ2, 20000)
+        y2, s2, n2 = o.integrate(a, o.init_ray(a, 1000.0, 120.0, al, -be), 1 / 32, 1.01 * o.horizon(a), 1010.0, o.STEP_EQ2, 20000)
+        assert s1 == s2 and n1 == n2
+        assert np.allclose(y1[[1, 3]], y2[[1, 3]], rtol=1e-9, atol=1e-9) and np.isclose(y1[2], np.pi - y2[2], atol=1e-9)
+        # spin flip: (a, alpha) -> (-a, -alpha) mirrors phi
+        y3, s3, n3 = o.integrate(-a, o.init_ray(-a, 1000.0, 60.0, -al, be), 1 / 32, 1.01 * o.horizon(a), 1010.0, o.STEP_EQ2, 20000)
+        assert s1 == s3 and n1 == n3
+        assert np.allclose(y1[[1, 2]], y3[[1, 2]], rtol=1e-9, atol=1e-9) and np.isclose(y1[3], -y3[3], atol=1e-8)
+
+
+def test_a0_rotation_invariance():
+    # Schwarzschild: with the REL rule (dlambda depends on r only) the radial motion depends on
+    # sqrt(alpha^2 + beta^2) only, up to the coordinate dependence of the RK4 truncation error,
+    # which must fall as h^4
+    spread = []
+    for h in (1 / 32, 1 / 64):
+        out = []
+        for ang in (0.3, 1.4, 2.9, 4.4):
+            y, s, n = o.integrate(0.0, o.init_ray(0.0, 1000.0, 60.0, 7.0 * np.cos(ang), 7.0 * np.sin(ang)),
+                                  h, 2.02, 1010.0, o.STEP_REL, 20000)
+            out.append((y[1], s, n))
+        assert all(s == o.ESCAPED for _, s, _ in out)
+        assert len({n for _, _, n in out}) == 1
+        spread.append(max(abs(r - out[0][0]) for r, _, _ in out) / out[0][0])
+    assert spread[0] < 2e-4 and spread[1] < spread[0] / 8, spread
+
+
+def test_conservation_along_rays():
+    # E, L_z, Q and the null norm between the first and last state (north_star); truncation-limited
+    # at h = 1/32 (reading R12)
+    a = 0.9
+    res = o.trace(a, 1000.0, 60.0, 10.0, 16, 16, rule=o.STEP_EQ2)
+    esc = res["status"] == o.ESCAPED
+    d = []
+    for y0, y in zip(res["y0"][esc], res["y"][esc]):
+        i0, i1 = o.invariants(a, y0), o.invariants(a, y)
+        d.append([abs(i1[0] - 1), abs(i1[1] - i0[1]) / max(abs(i0[1]), 0.1), abs(i1[2] - i0[2]) / abs(i0[2]), abs(i1[3])])
+    d = np.array(d)
+    assert np.median(d, axis=0).max() < 1e-6 and d.max() < 2e-4, (np.median(d, axis=0), d.max(axis=0))
+
+
+def test_pole_ray_value_printed_in_paper_is_the_face_on_critical_radius():
+    # r0 sin(theta0) = 4.833605 M for a = 0.99 "passes both the south and north poles ...
+    # and eventually hit[s] the event horizon": a ray parallel to the spin axis with L_z = 0 on the
+    # critical curve.  Closed form: xi(r_p) = 0, radius = sqrt(eta(r_p) + a^2).
+    from scipy.optimize import brentq
+    a = GOLD["pole_ray_spin"]
+    pro, ret = cf.photon_orbit_radii(a)
+    rp = brentq(lambda r: cf.xi_eta(a, r)[0], pro, ret)
+    radius = np.sqrt(cf.xi_eta(a, rp)[1] + a * a)
+    # the printed value lies 0.1 % inside that radius (4.838284): the ray winds "a couple times"
+    # and is captured, as P:93 says
+    assert 0 < radius - GOLD["pole_ray_impact"] < 1.1e-3 * radius
+    assert abs(radius - 4.838284) < 1e-6
+    # the oracle's nearly face-on (i = 1 deg) shadow edge brackets the closed-form curve, whose
+    # radius there is that value to 0.2 %: rays 1 % inside are captured, 1 % outside escape.
+    # (alpha = 0 exactly is avoided: such rays have |L_z| < 1e-5 and hit the pole failure the
+    # paper describes; its cure is SURVEY 8(f) NEXT-1.)
+    for ang in (0.0, 0.8, 2.0, np.pi):
+        rc = cf.bardeen_rho(a, 1.0, ang)
+        assert abs(rc / GOLD["pole_ray_impact"] - 1) < 3e-2
+        for f, want in ((0.99, o.CAPTURED), (1.01, o.ESCAPED)):
+            y0 = o.init_ray(a, GOLD["image_plane_radius"], 1.0, f * rc * np.cos(ang), f * rc * np.sin(ang))
+            _, st, _ = o.integrate(a, y0, GOLD["step_parameter"], 1.01 * o.horizon(a), 1010.0, o.STEP_EQ2, 20000)
+            assert st == want
+
+
+def _paper_fit(a, inc_deg):
+    R0 = sum(c * a ** k for k, c in enumerate(GOLD["fit_R0_coeffs"]))
+    c1 = GOLD["fit_R1_coeffs"]
+    R1 = (c1[0] - c1[1] / ((a - c1[2]) ** 2 + c1[3])) * 1e-3
+    ph = GOLD["fit_R_phase"]
+    R = R0 + R1 * np.cos(np.deg2rad(ph[0] * inc_deg - ph[1]))
+    ca = GOLD["fit_A0_coeffs"]
+    A0 = ca[0] * a ** ca[1] + ca[2] * a ** ca[3] + ca[4] * a ** ca[5]
+    cn = GOLD["fit_n_coeffs"]
+    n = cn[0] * (1 - a) ** cn[1] + cn[2] * (1 - a) ** cn[3]
+    return R, A0 * np.sin(np.deg2rad(inc_deg)) ** n
+
+
+@pytest.mark.parametrize("a,inc", [(0.0, 60.0), (0.9, 60.0), (0.99, 90.0)])
+def test_shadow_stats_against_bardeen_and_paper_fits(a, inc):
+    # eqs. (6)-(8) of the paper evaluated on the oracle's capture map vs the closed-form curve
+    n, W = 96, 10.0
+    res = o.trace(a, 1000.0, inc, W, n, n, rule=o.STEP_EQ2, threads=4, want_y0=False)
+    cmap = (res["status"] == o.CAPTURED).reshape(n, n).astype(np.uint8)
+    st, radius = o.shadow_stats(cmap, W, 360)
+    ex = cf.bardeen_stats(a, inc)
+    px = 2 * W / n
+    assert abs(st["area"] - ex["area"]) < 0.012 * ex["area"]
+    assert abs(st["alpha_min"] - ex["alpha_min"]) < px and abs(st["alpha_max"] - ex["alpha_max"]) < px
+    assert abs(st["D"] - ex["D"]) < px
+    assert abs(st["R_mean"] - ex["R_mean"]) < 0.5 * px
+    # pixelisation adds ~px/sqrt(12) of scatter to every spoke radius, i.e. ~0.58 px to A = 2 std(R)
+    assert abs(st["A"] - ex["A"]) < 0.8 * px
+    assert abs(st["centroid_beta"]) < 1e-9 or abs(st["centroid_beta"]) < px
+    vt = 2 * np.pi * (np.arange(360) + 0.5) / 360
+    assert np.max(np.abs(radius - cf.bardeen_rho(a, inc, vt))) < 1.1 * px
+    # the paper's fitting formulae, eqs. (11)-(14): soft (they are fits)
+    Rf, Af = _paper_fit(a, inc)
+    assert abs(ex["R_mean"] - Rf) < 0.04 and abs(ex["A"] - Af) < 0.03
+    assert abs(st["R_mean"] - Rf) < 0.04 + 0.5 * px
+
+
+def test_shadow_stats_on_synthetic_disc():
+    # exact geometry: a disc of radius 3 centred at (1, 0)
+    n, W = 400, 8.0
+    al, be = _grid(W, n, n)
+    cmap = (np.hypot(al - 1.0, be) < 3.0).reshape(n, n).astype(np.uint8)
+    st, radius = o.shadow_stats(cmap, W, 720)
+    px = 2 * W / n
+    assert abs(st["area"] - np.pi * 9) < 0.01 * np.pi * 9
+    assert abs(st["centroid_alpha"] - 1.0) < 1e-3 and abs(st["centroid_beta"]) < 1e-9
+    assert abs(st["alpha_min"] + 2.0) < px and abs(st["alpha_max"] - 4.0) < px
+    assert abs(st["D"] - 1.0) < px and abs(st["R_mean"] - 3.0) < 0.5 * px and st["A"] < px
+    vt = 2 * np.pi * (np.arange(720) + 0.5) / 720
+    rho = np.cos(vt) + np.sqrt(9 - np.sin(vt) ** 2)        # boundary of the disc seen from the origin
+    assert np.max(np.abs(radius - rho)) < 1.5 * px
+    # empty map
+    st0, r0 = o.shadow_stats(np.zeros((8, 8), np.uint8), 1.0, 16)
+    assert st0["area"] == 0 and st0["n_captured"] == 0 and np.all(r0 == 0)
+
+
+def test_op_tally_is_stable_and_plausible():
+    a = 0.7
+    y = o.init_ray(a, 1000.0, 45.0, 3.0, 4.0)
+    t = o.op_tally(a, y, 1 / 32, o.STEP_REL)
+    t2 = o.op_tally(a, o.init_ray(a, 1000.0, 45.0, -9.0, 1.0), 1 / 32, o.STEP_REL)
+    assert t == t2                                   # straight-line code: state-independent
+    assert t["sin"] == 4 and t["cos"] == 4           # four RHS evaluations per RK4 step
+    flops = t["add"] + t["mul"] + t["div"] + t["sqrt"] + t["sin"] + t["cos"]
+    assert 600 < flops < 900
+    te = o.op_tally(a, y, 1 / 32, o.STEP_EQ2)
+    assert te["div"] > t["div"] and te["sqrt"] == 1
