@@ -1,0 +1,203 @@
+/* gray.h — C ABI of libgray: photon null geodesics in Kerr spacetime on one B200 (sm_100a).
+ *
+ * The hot path of GRay (Chan, Psaltis & Ozel, arXiv 1303.5057; P:<n> = PAPER.md line n):
+ * "integrate the second-order geodesic equations" for very many independent photons
+ * with a 4th-order Runge-Kutta scheme from an image plane at r = 1000 M
+ * until each ray reaches the horizon r_bh = 1 + sqrt(1 - a^2) or
+ * leaves; then read the shadow / photon ring off the capture map (eqs. 6-8).
+ *
+ * Conventions
+ *   units           G = c = M = 1 (lengths in gravitational radii)
+ *   coordinates     Boyer-Lindquist (t, r, theta, phi); state of a photon = x^mu and k^mu = dx^mu/dlambda
+ *   memory          every pointer named *_dev is DEVICE memory owned by the caller (PyTorch tensors in
+ *                   the Python binding); the library never allocates, frees or keeps it.  Pointers
+ *                   named *_host are HOST memory owned by the caller.
+ *   layout          structure of arrays of 16-byte-aligned 4-vectors: x[p] = (t, r, theta, phi),
+ *                   k[p] = (k^t, k^r, k^theta, k^phi); float4 for GRAY_F32, 4 doubles for GRAY_F64.
+ *   stream          `cuda_stream` is a cudaStream_t passed as void* (NULL = the default stream).  All
+ *                   work is enqueued on it.  Functions that return values to *_host pointers
+ *                   synchronise that stream before returning and say so below; the others are
+ *                   asynchronous.
+ *   errors          every function returns GRAY_OK (0) or a negative gray_status and never throws or
+ *                   exits; gray_last_error() gives a thread-local message.  Argument errors are
+ *                   detected before any launch.  A ray whose state goes non-finite is data, not an
+ *                   error: its status becomes GRAY_BAD.
+ *   no fallback     there is no CPU path: without a CUDA device every compute entry point returns
+ *                   GRAY_ERR_CUDA.
+ */
+#ifndef GRAY_H_
+#define GRAY_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define GRAY_API __attribute__((visibility("default")))
+#else
+#define GRAY_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  GRAY_OK = 0,
+  GRAY_ERR_ARG = -1,         /* null / misaligned pointer, size mismatch, bad enum                  */
+  GRAY_ERR_DOMAIN = -2,      /* |a| >= 1, r_obs <= 0, half_width <= 0, h <= 0, inclination out of [0,180] */
+  GRAY_ERR_WORKSPACE = -3,   /* workspace missing or smaller than gray_workspace_bytes()            */
+  GRAY_ERR_CUDA = -4,        /* CUDA runtime error (message in gray_last_error)                     */
+  GRAY_ERR_UNSUPPORTED = -5
+} gray_status;
+
+typedef enum { GRAY_F32 = 0, GRAY_F64 = 1 } gray_prec;
+
+/* Step-size rule, evaluated at the start of each step and frozen over its four stages; negative
+ * because rays are traced backwards from the observer.
+ *   GRAY_STEP_REL  dlambda = -h r                              (BASELINE.json configs, literal)
+ *   GRAY_STEP_EQ2  dlambda = -min( h / (|k^r|/r + |k^theta| + |k^phi|), (r - r_bh) / (2 |k^r|) )
+ *                  paper eq. (2), with its Delta := h ~ 1/32                          */
+typedef enum { GRAY_STEP_REL = 0, GRAY_STEP_EQ2 = 1 } gray_step_rule;
+
+typedef enum { GRAY_LIVE = 0, GRAY_CAPTURED = 1, GRAY_ESCAPED = 2, GRAY_BAD = 3 } gray_ray_status;
+
+/* How photons are mapped to threads by gray_integrate.
+ *   GRAY_SCHED_REFILL  persistent warps; a lane whose photon has terminated fetches the next live
+ *                      photon from a device-side queue, so warps stay full (in-register stream
+ *                      compaction driven by __ballot_sync masks).  Default.
+ *   GRAY_SCHED_STATIC  photon p on thread p for the whole call, a warp leaves when all its lanes are
+ *                      done (the paper's fixed grid; kept for comparison).
+ * Per-photon results are bit-identical for both and for any refill_interval.                       */
+typedef enum { GRAY_SCHED_REFILL = 0, GRAY_SCHED_STATIC = 1 } gray_schedule;
+
+typedef enum { GRAY_PIXELS_GRID = 0, GRAY_PIXELS_RANDOM = 1 } gray_pixels;
+
+/* A batch of photons.  The caller fills the four pointers, n and prec; gray_init_rays* fills the
+ * rest (the description of the image plane), which gray_integrate / gray_classify /
+ * gray_shadow_edge read.  x and k must be 16-byte aligned.                                          */
+typedef struct {
+  void* x_dev;            /* n x 4 scalars (t, r, theta, phi)                                        */
+  void* k_dev;            /* n x 4 scalars (k^t, k^r, k^theta, k^phi)                                */
+  uint8_t* status_dev;    /* n x gray_ray_status                                                     */
+  uint32_t* steps_dev;    /* n x RK4 steps taken so far                                              */
+  uint64_t n;             /* photons held by these buffers                                           */
+  int32_t prec;           /* gray_prec                                                               */
+  int32_t pixels;         /* gray_pixels                                                             */
+  double a;               /* spin, |a| < 1                                                    */
+  double r_obs;           /* distance of the image plane, 1000 M in the paper               */
+  double inc_deg;         /* observer inclination i in degrees from the spin axis            */
+  double half_width;      /* image plane covers alpha, beta in [-half_width, half_width]             */
+  int32_t nx, ny;         /* grid workload: pixels per row (alpha, fast) and rows (beta, slow)       */
+  uint64_t seed;          /* random workload: key of the counter-based pixel generator               */
+  uint64_t p0;            /* global index of photon 0 of this batch (sharding across GPUs / chunks)  */
+} gray_state;
+
+/* Image plane -> initial photon states ("initial conditions ... as in Psaltis & Johannsen
+ * (2012)"; readings R1-R4).  One thread per photon, fp64 arithmetic, rounded to
+ * state->prec on store.  Photon j of the batch is global photon p = p0 + j:
+ *   grid    pixel centre alpha = -W + (col + 1/2) 2W/nx, beta = -W + (row + 1/2) 2W/ny,
+ *           col = p mod nx, row = p / nx; requires p0 + n <= nx * ny
+ *   random  (alpha, beta) from the stateless generator of DESIGN.md keyed by (seed, p)
+ *   position  r_obs o + alpha yhat + beta bhat,  o = (sin i, 0, cos i), bhat = (-cos i, 0, sin i)
+ *   momentum  along +o, k^t from the null condition g_mu_nu k^mu k^nu = 0, normalised to E = -k_t = 1
+ * Writes x, k, status = GRAY_LIVE, steps = 0 and the image-plane fields of *state.  Asynchronous.
+ * Errors: GRAY_ERR_ARG, GRAY_ERR_DOMAIN (also when half_width is so large that a pixel starts
+ * outside 1.01 r_obs), GRAY_ERR_CUDA.                                                               */
+GRAY_API int gray_init_rays(gray_state* state, double a, double r_obs, double inc_deg, double half_width,
+                   int32_t nx, int32_t ny, uint64_t p0, void* cuda_stream);
+GRAY_API int gray_init_rays_random(gray_state* state, double a, double r_obs, double inc_deg, double half_width,
+                          uint64_t seed, uint64_t p0, void* cuda_stream);
+
+typedef struct {
+  double h;                  /* step parameter, the paper's Delta ~ 1/32                      */
+  double r_capture_factor;   /* captured when r < factor * r_bh (configs: 1.01); if 0, the paper's    */
+  double horizon_delta;      /*   r < r_bh + horizon_delta (delta ~ 1e-6) is used instead       */
+  double r_escape_factor;    /* escaped when r > factor * r_obs (configs: 1.01)                       */
+  int32_t rule;              /* gray_step_rule                                                        */
+  int32_t schedule;          /* gray_schedule                                                         */
+  int32_t refill_interval;   /* REFILL: RK4 steps between looks at the termination mask (>= 1; 0 = default) */
+  int32_t frozen;            /* peak-rate case of BASELINE config 4 (reading R17): every
+                                live photon is stepped until its counter reaches max_steps with no
+                                early exit; once a test fires its state, status and step count are
+                                frozen by select while the arithmetic continues                      */
+} gray_step_params;
+
+/* Bytes of device workspace gray_integrate / gray_classify / gray_shadow_edge need (queue head and
+ * counters; independent of n today, the argument is kept for layouts that are not).                */
+GRAY_API size_t gray_workspace_bytes(uint64_t n);
+
+/* Integrate photons 0 .. n_photons-1 of the batch (n_photons <= state->n) whose status is GRAY_LIVE:
+ * repeat { dlambda by the step rule; one classical RK4 step of the 8 equations dx^mu/dlambda = k^mu,
+ * dk^mu/dlambda = -Gamma^mu_ab k^a k^b; theta remap of eq. (3); steps += 1; tests in the
+ * order non-finite -> GRAY_BAD, r < r_capture -> GRAY_CAPTURED, r > r_escape -> GRAY_ESCAPED } until a
+ * test fires or steps == max_steps (the photon then stays GRAY_LIVE and a later call resumes it).  The
+ * stored state is the first one that satisfies a test.  x, k, status, steps are updated in place.
+ * Asynchronous.  Counters of the call are left in the workspace for gray_integrate_counters().
+ * Errors: GRAY_ERR_ARG, GRAY_ERR_DOMAIN, GRAY_ERR_WORKSPACE, GRAY_ERR_CUDA.                         */
+GRAY_API int gray_integrate(gray_state* state, uint64_t n_photons, uint32_t max_steps,
+                   const gray_step_params* params, void* workspace_dev, size_t workspace_bytes,
+                   void* cuda_stream);
+
+typedef struct {
+  uint64_t photon_steps;     /* RK4 steps that advanced a live photon (the unit of BASELINE's metric)  */
+  uint64_t issued_steps;     /* lane-steps issued by warps, including idle and frozen lanes            */
+  uint64_t photons_done;     /* photons this call brought to CAPTURED / ESCAPED / BAD                  */
+  uint64_t photons_live;     /* photons this call left LIVE at max_steps                               */
+} gray_counters;
+
+/* Counters of the last gray_integrate on this workspace.  Synchronises the stream.                  */
+GRAY_API int gray_integrate_counters(const void* workspace_dev, gray_counters* counters_host, void* cuda_stream);
+
+/* Per-pixel capture flags (capture_map[p] = 1 iff status[p] == GRAY_CAPTURED, else 0; may be NULL)
+ * and the number of photons in each gray_ray_status (counts_host[4]).  Synchronises the stream.     */
+GRAY_API int gray_classify(const gray_state* state, uint8_t* capture_map_dev, uint64_t counts_host[4],
+                  void* workspace_dev, size_t workspace_bytes, void* cuda_stream);
+
+/* Shadow / photon-ring statistics of a grid image (reading R13):
+ *   area = N_captured dalpha dbeta; centroid = mean (alpha, beta) of captured pixel centres;
+ *   alpha_min / alpha_max = outer edges of the extreme captured columns; D = |alpha_min + alpha_max| / 2
+ *   (eq. 6); rho(vartheta_k), k = 0 .. n_angles-1, vartheta_k = 2 pi (k + 1/2) / n_angles about the image
+ *   origin: marching outwards in steps of half a pixel, the mid-point between the last sample whose
+ *   pixel is captured and the first whose pixel is not; R_k = distance of that point from
+ *   ((alpha_min + alpha_max)/2, 0); R_mean = mean R_k (eq. 7); A = 2 std R_k (eq. 8).                */
+typedef struct {
+  double area, centroid_alpha, centroid_beta, alpha_min, alpha_max, D, R_mean, A;
+  uint64_t n_captured;
+} gray_shadow_stats;
+
+/* Requires a full grid batch (pixels == GRAY_PIXELS_GRID, p0 == 0, n == nx * ny).  radius_dev
+ * (n_angles doubles) may be NULL.  Synchronises the stream.                                         */
+GRAY_API int gray_shadow_edge(const gray_state* state, int32_t n_angles, double* radius_dev,
+                     gray_shadow_stats* stats_host, void* workspace_dev, size_t workspace_bytes,
+                     void* cuda_stream);
+
+/* End-to-end variant with HOST buffers (bench.py's `e2e` figure).  n photons whose initial states are
+ * x_in_host / k_in_host (n x 4 scalars of `prec`, status LIVE, steps 0 implied) are streamed through
+ * the GPU in chunks of `chunk` photons on two internal streams, so that the host->device copy of one
+ * chunk and the device->host copy of another overlap the integration of a third: copy in, gray_integrate
+ * semantics with (a, r_obs, params, max_steps), copy out.  Results: x_out_host, k_out_host (may alias the
+ * inputs), status_host (n bytes), steps_host (n).  Host buffers should be pinned (cudaHostAlloc /
+ * torch pin_memory) for the copies to be asynchronous.  scratch_dev must hold
+ * gray_host_scratch_bytes(chunk, prec) bytes of device memory, 256-byte aligned.  counters_host (may be
+ * NULL) receives the summed gray_counters.  Synchronous: returns when every result is in host memory. */
+GRAY_API size_t gray_host_scratch_bytes(uint64_t chunk, int32_t prec);
+GRAY_API int gray_integrate_host(const void* x_in_host, const void* k_in_host, void* x_out_host, void* k_out_host,
+                        uint8_t* status_host, uint32_t* steps_host, uint64_t n, int32_t prec, double a,
+                        double r_obs, uint32_t max_steps, const gray_step_params* params, uint64_t chunk,
+                        void* scratch_dev, size_t scratch_bytes, gray_counters* counters_host);
+
+/* Register-only FFMA (GRAY_F32) or DFMA (GRAY_F64) microbenchmark: the measured CUDA-core peak the
+ * integrator's rate is divided by.  Runs `iters` dependent-chain-free FMA rounds
+ * on every SM, times them with CUDA events on the stream, returns FLOP/s (FMA = 2).  Synchronises.  */
+GRAY_API int gray_fma_peak(int32_t prec, int32_t iters, double* flops_per_s_host, void* cuda_stream);
+
+/* Device facts used by the benchmark: SM count and SM clock (kHz) reported by the runtime.         */
+GRAY_API int gray_device_info(int32_t* sm_count_host, int32_t* sm_clock_khz_host);
+
+GRAY_API const char* gray_last_error(void);   /* thread-local, valid until the next call on this thread       */
+GRAY_API const char* gray_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GRAY_H_ */

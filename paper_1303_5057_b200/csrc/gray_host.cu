@@ -1,0 +1,102 @@
+// gray_host.cu — gray_integrate_host (include/gray.h): host buffers in, host buffers out, chunks
+// double-buffered over two streams so PCIe copies overlap the integrator kernel.
+#include "gray_internal.h"
+
+namespace gray {
+
+struct Slot {
+  char* x; char* k; uint32_t* steps; uint8_t* status; Workspace* ws;
+  cudaStream_t stream;
+  unsigned long long* c;     // counters of the chunk last run on this slot (pinned host staging)
+};
+
+static size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
+
+static size_t slot_bytes(uint64_t chunk, int prec) {
+  const size_t vec = (prec == GRAY_F32 ? 16 : 32);
+  return align256(chunk * vec) * 2 + align256(chunk * 4) + align256(chunk) + align256(sizeof(Workspace));
+}
+
+}  // namespace gray
+
+extern "C" {
+
+size_t gray_host_scratch_bytes(uint64_t chunk, int32_t prec) { return 2 * gray::slot_bytes(chunk, prec); }
+
+int gray_integrate_host(const void* x_in_host, const void* k_in_host, void* x_out_host, void* k_out_host,
+                        uint8_t* status_host, uint32_t* steps_host, uint64_t n, int32_t prec, double a, double r_obs,
+                        uint32_t max_steps, const gray_step_params* params, uint64_t chunk, void* scratch_dev,
+                        size_t scratch_bytes, gray_counters* counters_host) {
+  using namespace gray;
+  if (prec != GRAY_F32 && prec != GRAY_F64) { set_error("bad precision"); return GRAY_ERR_ARG; }
+  if (!params) { set_error("params is NULL"); return GRAY_ERR_ARG; }
+  if (counters_host) *counters_host = gray_counters{0, 0, 0, 0};
+  if (n == 0) return GRAY_OK;
+  if (!x_in_host || !k_in_host || !x_out_host || !k_out_host || !status_host || !steps_host) { set_error("NULL host buffer"); return GRAY_ERR_ARG; }
+  if (chunk == 0) { set_error("chunk must be positive"); return GRAY_ERR_ARG; }
+  if (chunk > n) chunk = n;
+  if (!scratch_dev || ((uintptr_t)scratch_dev & 255) || scratch_bytes < gray_host_scratch_bytes(chunk, prec)) {
+    set_error("scratch_dev is NULL, not 256-byte aligned or smaller than gray_host_scratch_bytes()");
+    return GRAY_ERR_WORKSPACE;
+  }
+  const size_t vec = (prec == GRAY_F32 ? 16 : 32);
+  Slot slot[2];
+  char* base = (char*)scratch_dev;
+  unsigned long long* pinned = nullptr;   // 2 x 4 counters; pinned so the copies back stay asynchronous
+  GRAY_CUDA(cudaHostAlloc(&pinned, 8 * sizeof(unsigned long long), cudaHostAllocDefault));
+  for (int s = 0; s < 2; ++s) {
+    char* p = base + s * slot_bytes(chunk, prec);
+    slot[s].x = p; p += align256(chunk * vec);
+    slot[s].k = p; p += align256(chunk * vec);
+    slot[s].steps = (uint32_t*)p; p += align256(chunk * 4);
+    slot[s].status = (uint8_t*)p; p += align256(chunk);
+    slot[s].ws = (Workspace*)p;
+    slot[s].c = pinned + 4 * s;
+    GRAY_CUDA(cudaStreamCreateWithFlags(&slot[s].stream, cudaStreamNonBlocking));
+  }
+  int rc = GRAY_OK;
+  gray_counters total = {0, 0, 0, 0};
+  uint64_t done_chunks = 0;
+  auto drain = [&](int s) -> int {   // wait for the chunk in flight on slot s and add its counters
+    GRAY_CUDA(cudaStreamSynchronize(slot[s].stream));
+    total.photon_steps += slot[s].c[0]; total.issued_steps += slot[s].c[1];
+    total.photons_done += slot[s].c[2]; total.photons_live += slot[s].c[3];
+    return GRAY_OK;
+  };
+  for (uint64_t lo = 0; lo < n && rc == GRAY_OK; lo += chunk, ++done_chunks) {
+    const int s = (int)(done_chunks & 1);
+    const uint64_t m = (n - lo < chunk) ? n - lo : chunk;
+    Slot& S = slot[s];
+    if (done_chunks >= 2) { rc = drain(s); if (rc) break; }
+    cudaError_t e;
+    e = cudaMemcpyAsync(S.x, (const char*)x_in_host + lo * vec, m * vec, cudaMemcpyHostToDevice, S.stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(S.k, (const char*)k_in_host + lo * vec, m * vec, cudaMemcpyHostToDevice, S.stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(S.status, GRAY_LIVE, m, S.stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(S.steps, 0, m * 4, S.stream);
+    if (e != cudaSuccess) { rc = cuda_fail(e, "gray_integrate_host: copy in"); break; }
+    gray_state st;
+    st.x_dev = S.x; st.k_dev = S.k; st.status_dev = S.status; st.steps_dev = S.steps;
+    st.n = m; st.prec = prec; st.pixels = GRAY_PIXELS_GRID;
+    st.a = a; st.r_obs = r_obs; st.inc_deg = 0; st.half_width = 0; st.nx = st.ny = 0; st.seed = 0; st.p0 = lo;
+    rc = gray_integrate(&st, m, max_steps, params, S.ws, sizeof(Workspace), S.stream);
+    if (rc) break;
+    e = cudaMemcpyAsync((char*)x_out_host + lo * vec, S.x, m * vec, cudaMemcpyDeviceToHost, S.stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync((char*)k_out_host + lo * vec, S.k, m * vec, cudaMemcpyDeviceToHost, S.stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(status_host + lo, S.status, m, cudaMemcpyDeviceToHost, S.stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(steps_host + lo, S.steps, m * 4, cudaMemcpyDeviceToHost, S.stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(S.c, &S.ws->photon_steps, 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, S.stream);
+    if (e != cudaSuccess) { rc = cuda_fail(e, "gray_integrate_host: copy out"); break; }
+  }
+  const uint64_t in_flight = done_chunks < 2 ? done_chunks : 2;
+  for (uint64_t q = 0; q < in_flight; ++q) {
+    const int s = (int)((done_chunks - 1 - q) & 1);
+    const int r2 = drain(s);
+    if (rc == GRAY_OK) rc = r2;
+  }
+  for (int s = 0; s < 2; ++s) cudaStreamDestroy(slot[s].stream);
+  cudaFreeHost(pinned);
+  if (counters_host) *counters_host = total;
+  return rc;
+}
+
+}  // extern "C"

@@ -1,0 +1,225 @@
+// gray_shadow.cu — gray_classify and gray_shadow_edge (include/gray.h): capture map, status counts and
+// the shadow / photon-ring statistics of paper eqs. (6)-(8), from the per-photon status.
+#include "gray_internal.h"
+
+namespace gray {
+
+__device__ __forceinline__ unsigned int warp_sum_u32(unsigned int v) { return __reduce_add_sync(0xffffffffu, v); }
+
+// status -> capture flags + histogram of the four statuses.  16 photons per thread per iteration when
+// the buffers allow 16-byte accesses.
+__global__ void __launch_bounds__(256) classify_kernel(const uint8_t* __restrict__ status, uint8_t* __restrict__ cmap,
+                                                       unsigned long long n, int vec_ok, Workspace* ws) {
+  unsigned int c[4] = {0, 0, 0, 0};
+  const unsigned long long tid = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const unsigned long long nthreads = (unsigned long long)gridDim.x * blockDim.x;
+  const unsigned long long nvec = vec_ok ? n / 16 : 0;
+  for (unsigned long long v = tid; v < nvec; v += nthreads) {
+    const uint4 w = ((const uint4*)status)[v];
+    const unsigned int in[4] = {w.x, w.y, w.z, w.w};
+    unsigned int out[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      unsigned int o = 0;
+#pragma unroll
+      for (int b = 0; b < 4; ++b) {
+        const unsigned int s = (in[q] >> (8 * b)) & 0xffu;
+        c[s & 3u] += 1u;
+        o |= (s == GRAY_CAPTURED ? 1u : 0u) << (8 * b);
+      }
+      out[q] = o;
+    }
+    if (cmap) ((uint4*)cmap)[v] = make_uint4(out[0], out[1], out[2], out[3]);
+  }
+  for (unsigned long long p = nvec * 16 + tid; p < n; p += nthreads) {
+    const unsigned int s = status[p];
+    c[s & 3u] += 1u;
+    if (cmap) cmap[p] = (s == GRAY_CAPTURED) ? 1 : 0;
+  }
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    const unsigned int t = warp_sum_u32(c[q]);
+    if ((threadIdx.x & 31) == 0 && t) atomicAdd(&ws->counts[q], (unsigned long long)t);
+  }
+}
+
+// captured pixels: count, sums of column / row indices (exact integers), extreme columns
+__global__ void __launch_bounds__(256) shadow_reduce_kernel(const uint8_t* __restrict__ status, unsigned long long n,
+                                                            unsigned int nx, Workspace* ws) {
+  unsigned long long cnt = 0, sc = 0, sr = 0;
+  unsigned int cmin = 0xffffffffu, cmax = 0;
+  const unsigned long long nthreads = (unsigned long long)gridDim.x * blockDim.x;
+  for (unsigned long long p = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += nthreads) {
+    if (status[p] == GRAY_CAPTURED) {
+      const unsigned int col = (unsigned int)(p % nx), row = (unsigned int)(p / nx);
+      ++cnt; sc += col; sr += row;
+      cmin = min(cmin, col); cmax = max(cmax, col);
+    }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+    sc += __shfl_xor_sync(0xffffffffu, sc, o);
+    sr += __shfl_xor_sync(0xffffffffu, sr, o);
+  }
+  cmin = __reduce_min_sync(0xffffffffu, cmin);
+  cmax = __reduce_max_sync(0xffffffffu, cmax);
+  if ((threadIdx.x & 31) == 0 && cnt) {
+    atomicAdd(&ws->n_captured, cnt);
+    atomicAdd(&ws->sum_col, sc);
+    atomicAdd(&ws->sum_row, sr);
+    atomicMin(&ws->min_col, cmin);
+    atomicMax(&ws->max_col, cmax);
+  }
+}
+
+struct EdgeArgs {
+  const uint8_t* status;
+  long long nx, ny;
+  double W;
+  int n_angles;
+  double* radius;
+  Workspace* ws;
+};
+
+// rho(vartheta): march outwards from the image origin in half-pixel steps until the pixel under the
+// sample is not captured (or the image ends); the edge is the mid-point of the last two samples.
+__device__ double spoke_radius(const EdgeArgs& A, double da, double db, double delta, double cv, double sv) {
+  for (long long j = 0;; ++j) {
+    const double q = (double)j * delta;
+    const long long col = (long long)floor((q * cv + A.W) / da);
+    const long long row = (long long)floor((q * sv + A.W) / db);
+    const bool inside = col >= 0 && col < A.nx && row >= 0 && row < A.ny;
+    if (!inside) return ((double)j - 0.5) * delta;
+    if (A.status[row * A.nx + col] != GRAY_CAPTURED) return j == 0 ? 0.0 : ((double)j - 0.5) * delta;
+  }
+}
+
+__device__ double block_sum(double v, double* sh) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  __syncthreads();
+  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = v;
+  __syncthreads();
+  double t = 0.0;
+  for (int w = 0; w < (int)(blockDim.x >> 5); ++w) t += sh[w];
+  return t;
+}
+
+// one block: spokes, then eqs. (6)-(8)
+__global__ void __launch_bounds__(1024) shadow_edge_kernel(const __grid_constant__ EdgeArgs A) {
+  __shared__ double sh[32];
+  Workspace* ws = A.ws;
+  const double da = 2.0 * A.W / (double)A.nx, db = 2.0 * A.W / (double)A.ny;
+  const double delta = fmin(da, db) / 2.0;
+  const unsigned long long ncap = ws->n_captured;
+  const double amin = ncap ? -A.W + (double)ws->min_col * da : 0.0;
+  const double amax = ncap ? -A.W + (double)(ws->max_col + 1) * da : 0.0;
+  const double centre = (amin + amax) / 2.0;
+  const double two_pi = 2.0 * 3.14159265358979323846;
+  double sumR = 0.0;
+  for (int k = threadIdx.x; k < A.n_angles; k += blockDim.x) {
+    const double vt = two_pi * ((double)k + 0.5) / (double)A.n_angles;
+    double sv, cv;
+    sincos(vt, &sv, &cv);
+    const double rho = spoke_radius(A, da, db, delta, cv, sv);
+    if (A.radius) A.radius[k] = rho;
+    const double x = rho * cv - centre, y = rho * sv;
+    sumR += sqrt(x * x + y * y);
+  }
+  const double mean = A.n_angles > 0 ? block_sum(sumR, sh) / (double)A.n_angles : 0.0;
+  double var = 0.0;
+  for (int k = threadIdx.x; k < A.n_angles; k += blockDim.x) {
+    const double vt = two_pi * ((double)k + 0.5) / (double)A.n_angles;
+    double sv, cv;
+    sincos(vt, &sv, &cv);
+    const double rho = spoke_radius(A, da, db, delta, cv, sv);
+    const double x = rho * cv - centre, y = rho * sv;
+    const double d = sqrt(x * x + y * y) - mean;
+    var += d * d;
+  }
+  var = A.n_angles > 0 ? block_sum(var, sh) / (double)A.n_angles : 0.0;
+  if (threadIdx.x == 0) {
+    ws->stats[0] = (double)ncap * da * db;
+    ws->stats[1] = ncap ? -A.W + ((double)ws->sum_col / (double)ncap + 0.5) * da : 0.0;
+    ws->stats[2] = ncap ? -A.W + ((double)ws->sum_row / (double)ncap + 0.5) * db : 0.0;
+    ws->stats[3] = amin;
+    ws->stats[4] = amax;
+    ws->stats[5] = fabs(amin + amax) / 2.0;
+    ws->stats[6] = mean;
+    ws->stats[7] = 2.0 * sqrt(var);
+  }
+}
+
+static unsigned int reduce_grid(unsigned long long n, unsigned long long per_thread) {
+  unsigned long long blocks = (n / per_thread + 255) / 256 + 1;
+  const unsigned long long cap = (unsigned long long)sm_count() * 16;
+  if (blocks > cap) blocks = cap;
+  return (unsigned int)(blocks ? blocks : 1);
+}
+
+}  // namespace gray
+
+extern "C" {
+
+int gray_classify(const gray_state* state, uint8_t* capture_map_dev, uint64_t counts_host[4], void* workspace_dev,
+                  size_t workspace_bytes, void* cuda_stream) {
+  using namespace gray;
+  int rc = check_state(state, false);
+  if (rc) return rc;
+  if (!counts_host) { set_error("counts_host is NULL"); return GRAY_ERR_ARG; }
+  rc = check_workspace(workspace_dev, workspace_bytes);
+  if (rc) return rc;
+  cudaStream_t stream = (cudaStream_t)cuda_stream;
+  Workspace* ws = (Workspace*)workspace_dev;
+  GRAY_CUDA(cudaMemsetAsync(&ws->counts[0], 0, sizeof ws->counts, stream));
+  if (state->n) {
+    const int vec_ok = (((uintptr_t)state->status_dev & 15) == 0) && (!capture_map_dev || ((uintptr_t)capture_map_dev & 15) == 0);
+    classify_kernel<<<reduce_grid(state->n, 16), 256, 0, stream>>>(state->status_dev, capture_map_dev, state->n, vec_ok, ws);
+    GRAY_CUDA(cudaGetLastError());
+  }
+  unsigned long long c[4];
+  GRAY_CUDA(cudaMemcpyAsync(c, &ws->counts[0], sizeof c, cudaMemcpyDeviceToHost, stream));
+  GRAY_CUDA(cudaStreamSynchronize(stream));
+  for (int q = 0; q < 4; ++q) counts_host[q] = c[q];
+  return GRAY_OK;
+}
+
+int gray_shadow_edge(const gray_state* state, int32_t n_angles, double* radius_dev, gray_shadow_stats* stats_host,
+                     void* workspace_dev, size_t workspace_bytes, void* cuda_stream) {
+  using namespace gray;
+  int rc = check_state(state, true);
+  if (rc) return rc;
+  if (!stats_host || n_angles < 0) { set_error("stats_host is NULL or n_angles < 0"); return GRAY_ERR_ARG; }
+  if (state->pixels != GRAY_PIXELS_GRID || state->p0 != 0 || state->nx <= 0 || state->ny <= 0 ||
+      state->n != (uint64_t)state->nx * (uint64_t)state->ny) {
+    set_error("gray_shadow_edge needs a full grid image (pixels = GRID, p0 = 0, n = nx * ny)");
+    return GRAY_ERR_ARG;
+  }
+  rc = check_workspace(workspace_dev, workspace_bytes);
+  if (rc) return rc;
+  cudaStream_t stream = (cudaStream_t)cuda_stream;
+  Workspace* ws = (Workspace*)workspace_dev;
+  // sum_col .. n_captured; min_col must start at the maximum
+  GRAY_CUDA(cudaMemsetAsync(&ws->sum_col, 0, (char*)&ws->pad3[0] - (char*)&ws->sum_col, stream));
+  GRAY_CUDA(cudaMemsetAsync(&ws->min_col, 0xff, sizeof ws->min_col, stream));
+  shadow_reduce_kernel<<<reduce_grid(state->n, 4), 256, 0, stream>>>(state->status_dev, state->n, (unsigned int)state->nx, ws);
+  GRAY_CUDA(cudaGetLastError());
+  EdgeArgs A;
+  A.status = state->status_dev; A.nx = state->nx; A.ny = state->ny; A.W = state->half_width;
+  A.n_angles = n_angles; A.radius = radius_dev; A.ws = ws;
+  shadow_edge_kernel<<<1, 1024, 0, stream>>>(A);
+  GRAY_CUDA(cudaGetLastError());
+  double s[8];
+  unsigned long long ncap = 0;
+  GRAY_CUDA(cudaMemcpyAsync(s, &ws->stats[0], sizeof s, cudaMemcpyDeviceToHost, stream));
+  GRAY_CUDA(cudaMemcpyAsync(&ncap, &ws->n_captured, sizeof ncap, cudaMemcpyDeviceToHost, stream));
+  GRAY_CUDA(cudaStreamSynchronize(stream));
+  stats_host->area = s[0]; stats_host->centroid_alpha = s[1]; stats_host->centroid_beta = s[2];
+  stats_host->alpha_min = s[3]; stats_host->alpha_max = s[4]; stats_host->D = s[5];
+  stats_host->R_mean = s[6]; stats_host->A = s[7];
+  stats_host->n_captured = ncap;
+  return GRAY_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,270 @@
+"""Parity of the CUDA path (through the C ABI) with the oracle, element by element (-m gpu)."""
+import numpy as np
+import pytest
+import torch
+
+import closed_forms as cf
+import oracle as o
+import paper_1303_5057_b200 as g
+from gpu_common import edge_band, gpu_state, grid_pixels, rel_err_final, upload_state
+from paper_1303_5057_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+# ------------------------------------------------------------------------------------ init
+@pytest.mark.parametrize("prec", [g.GRAY_F32, g.GRAY_F64])
+@pytest.mark.parametrize("a,inc,W,nx,ny", [(0.0, 60.0, 10.0, 64, 64), (0.99, 90.0, 12.0, 50, 37), (0.7, 135.0, 15.0, 33, 21)])
+def test_init_rays_grid_matches_oracle(prec, a, inc, W, nx, ny):
+    b = g.PhotonBatch(nx * ny, prec)
+    g.gray_init_rays(b, a, wl.R_OBS, inc, W, nx, ny)
+    y, st, n = gpu_state(b)
+    ref = o.trace(a, wl.R_OBS, inc, W, nx, ny, max_steps=0)["y0"]
+    assert np.all(st == g.LIVE) and np.all(n == 0)
+    # components that vanish by symmetry (k^theta on the beta = 0 row at i = 90 deg) are compared on the
+    # scale of their column
+    col = np.abs(ref).max(axis=0, keepdims=True)
+    if prec == g.GRAY_F64:
+        # same formulas in a different order and another libm: a few ulp
+        assert np.all(np.abs(y - ref) <= 1e-13 * np.abs(ref) + 1e-15 * col)
+    else:
+        ref32 = ref.astype(np.float32).astype(np.float64)
+        assert np.all(np.abs(y - ref32) <= 1.2e-7 * np.abs(ref32) + 1e-9 * col)     # at most 1 fp32 ulp
+        assert np.mean(y == ref32) > 0.995
+
+
+@pytest.mark.parametrize("prec", [g.GRAY_F32, g.GRAY_F64])
+def test_init_rays_random_and_sharded_matches_oracle(prec):
+    c4 = wl.C4
+    n, p0 = 5000, 123456789012
+    b = g.PhotonBatch(n, prec)
+    g.gray_init_rays_random(b, c4["a"], wl.R_OBS, c4["inc_deg"], c4["half_width"], c4["seed"], p0)
+    y, _, _ = gpu_state(b)
+    idx = np.arange(p0, p0 + n, dtype=np.uint64)
+    ref = o.trace(c4["a"], wl.R_OBS, c4["inc_deg"], c4["half_width"], 0, 0, seed=c4["seed"], idx=idx, max_steps=0)["y0"]
+    tol = 1e-13 if prec == g.GRAY_F64 else 1.2e-7
+    if prec == g.GRAY_F32:
+        ref = ref.astype(np.float32).astype(np.float64)
+    assert np.all(np.abs(y - ref) <= tol * np.abs(ref) + 1e-2 * tol * np.abs(ref).max(axis=0, keepdims=True))
+    # grid sharding: photons [p0, p0 + n) of a larger image
+    b2 = g.PhotonBatch(1000, prec)
+    g.gray_init_rays(b2, 0.9, wl.R_OBS, 60.0, 10.0, 512, 512, p0=77777)
+    y2, _, _ = gpu_state(b2)
+    ref2 = o.trace(0.9, wl.R_OBS, 60.0, 10.0, 512, 512, idx=np.arange(77777, 78777, dtype=np.uint64), max_steps=0)["y0"]
+    if prec == g.GRAY_F32:
+        ref2 = ref2.astype(np.float32).astype(np.float64)
+    assert np.all(np.abs(y2 - ref2) <= tol * np.abs(ref2) + 1e-2 * tol * np.abs(ref2).max(axis=0, keepdims=True))
+
+
+# ------------------------------------------------------------------------------- integrate
+def _run_gpu_from_oracle_init(a, inc, W, nx, ny, prec, rule, **kw):
+    ref0 = o.trace(a, wl.R_OBS, inc, W, nx, ny, max_steps=0)["y0"]
+    b = g.PhotonBatch(nx * ny, prec)
+    upload_state(b, ref0)
+    b.set_image_plane(a, wl.R_OBS, inc, W, nx, ny)
+    g.gray_integrate(b, max_steps=wl.MAX_STEPS, params=g.StepParams(rule=rule, **kw))
+    return b
+
+
+@pytest.mark.parametrize("a,inc,W,nx,ny,rule", [
+    (0.0, 60.0, 10.0, 64, 64, g.STEP_EQ2),        # C1
+    (0.0, 60.0, 10.0, 64, 64, g.STEP_REL),        # C1 with the configs' literal rule
+    (0.9, 60.0, 10.0, 61, 45, g.STEP_EQ2),        # C2 geometry, ragged size (2745 = 21 blocks + 57)
+    (0.99, 90.0, 12.0, 48, 48, g.STEP_EQ2),       # C3 geometry
+])
+def test_integrate_f64_matches_oracle(a, inc, W, nx, ny, rule):
+    # north_star: "fp64 GPU vs oracle: <= 1e-9 relative"
+    b = _run_gpu_from_oracle_init(a, inc, W, nx, ny, g.GRAY_F64, rule)
+    y, st, n = gpu_state(b)
+    ref = o.trace(a, wl.R_OBS, inc, W, nx, ny, rule=rule, threads=8)
+    al, be = grid_pixels(W, nx, ny)
+    band = edge_band(a, inc, al, be)
+    same = (st == ref["status"]) & (n == ref["steps"])
+    assert np.all(same | band), np.flatnonzero(~same & ~band)[:10]
+    assert same.mean() >= 0.999
+    fin = same & (ref["status"] != o.BAD)
+    err = np.abs(y[fin] - ref["y"][fin]) / np.maximum(np.abs(ref["y"][fin]), 1.0)
+    # the arithmetic is the same algorithm in a different association order: errors are rounding
+    # noise amplified along the ray; 1e-9 away from the critical curve
+    assert err[~band[fin]].max() <= 1e-9, err[~band[fin]].max()
+    counts = g.gray_classify(b)
+    assert counts == [int((st == s).sum()) for s in range(4)]
+
+
+@pytest.mark.parametrize("a,inc,W,nx,ny", [(0.0, 60.0, 10.0, 64, 64), (0.9, 60.0, 10.0, 64, 64), (0.99, 90.0, 12.0, 64, 64),
+                                           (0.7, 45.0, 15.0, 64, 64)])
+def test_integrate_f32_matches_fp64_oracle(a, inc, W, nx, ny):
+    # north_star tolerances for fp32 GPU vs fp64 oracle, protocol of DESIGN.md reading R11
+    b = g.PhotonBatch(nx * ny, g.GRAY_F32)
+    g.gray_init_rays(b, a, wl.R_OBS, inc, W, nx, ny)
+    y0, _, _ = gpu_state(b)
+    g.gray_integrate(b, max_steps=wl.MAX_STEPS, params=g.StepParams(rule=g.STEP_EQ2))
+    y, st, n = gpu_state(b)
+    ref = o.trace(a, wl.R_OBS, inc, W, nx, ny, rule=o.STEP_EQ2, init_f32=True, threads=8)
+    assert np.array_equal(ref["y0"], y0) or np.mean(ref["y0"] == y0) > 0.999
+    al, be = grid_pixels(W, nx, ny)
+    band = edge_band(a, inc, al, be)
+    # (i) classification: >= 99.9 % agree, every mismatch within 1 % of the critical curve
+    mism = st != ref["status"]
+    assert mism.mean() <= 1e-3 and np.all(band[mism])
+    assert not np.any(st == g.LIVE)
+    # exact classifier, too
+    exact = np.array([cf.captured_exact(a, *(lambda i: (i[1] / i[0], i[2] / i[0] ** 2))(o.invariants(a, v))) for v in ref["y0"]])
+    assert np.all(((st == g.CAPTURED) == exact) | band)
+    # (ii)/(iii) final (r, theta, phi) at equal step count
+    diff = np.flatnonzero((n != ref["steps"]) & ~mism)
+    assert diff.size <= 0.01 * n.size
+    yref = ref["y"].copy()
+    if diff.size:
+        forced = o.trace(a, wl.R_OBS, inc, W, nx, ny, idx=diff.astype(np.uint64), rule=o.STEP_EQ2, init_f32=True,
+                         force_steps=n[diff])
+        yref[diff] = forced["y"]
+    ok = ~band & ~mism
+    # pole band (reading R14): rays passing within ~1e-2 rad of the axis are reported, not bounded
+    pole = np.abs(al * np.sin(np.deg2rad(inc))) < 0.05
+    err = rel_err_final(y[ok & ~pole], yref[ok & ~pole])
+    assert np.quantile(err, 0.99) <= 2e-4
+    assert err.max() <= 1e-3, (err.max(), np.sum(err > 1e-3))
+
+
+def test_schedules_intervals_and_resume_are_bit_identical():
+    a, inc, W, nx, ny = 0.9, 60.0, 10.0, 96, 51
+    outs = []
+    for prec in (g.GRAY_F32, g.GRAY_F64):
+        base = None
+        for kw in (dict(schedule=g.SCHED_REFILL, refill_interval=8), dict(schedule=g.SCHED_REFILL, refill_interval=1),
+                   dict(schedule=g.SCHED_REFILL, refill_interval=37), dict(schedule=g.SCHED_STATIC)):
+            b = g.PhotonBatch(nx * ny, prec)
+            g.gray_init_rays(b, a, wl.R_OBS, inc, W, nx, ny)
+            g.gray_integrate(b, max_steps=wl.MAX_STEPS, params=g.StepParams(rule=g.STEP_EQ2, **kw))
+            cur = (b.x.clone(), b.k.clone(), b.status.clone(), b.steps.clone())
+            cnt = g.gray_integrate_counters(b)
+            assert cnt["photon_steps"] == int(b.steps.sum().item()) and cnt["photons_done"] == nx * ny
+            assert cnt["issued_steps"] >= cnt["photon_steps"]
+            if base is None:
+                base = cur
+            else:
+                assert all(torch.equal(u.view(torch.uint8), v.view(torch.uint8)) for u, v in zip(base, cur)), kw
+        # resume: 100 steps, then 250 more, then to the end == one uninterrupted call
+        b = g.PhotonBatch(nx * ny, prec)
+        g.gray_init_rays(b, a, wl.R_OBS, inc, W, nx, ny)
+        total = 0
+        for cap in (100, 350, wl.MAX_STEPS):
+            g.gray_integrate(b, max_steps=cap, params=g.StepParams(rule=g.STEP_EQ2))
+            c = g.gray_integrate_counters(b)
+            total += c["photon_steps"]
+            if cap == 100:
+                assert c["photons_live"] == nx * ny and c["photon_steps"] == 100 * nx * ny
+                assert int(b.steps.min().item()) == 100 and g.gray_classify(b)[g.LIVE] == nx * ny
+        cur = (b.x, b.k, b.status, b.steps)
+        assert all(torch.equal(u.view(torch.uint8), v.view(torch.uint8)) for u, v in zip(base, cur))
+        assert total == int(b.steps.sum().item())
+
+
+@pytest.mark.parametrize("prec", [g.GRAY_F32, g.GRAY_F64])
+def test_frozen_peak_rate_mode_matches_oracle(prec):
+    # BASELINE config C4 peak case, reading R17: 1000 REL steps for every lane, state frozen by select
+    c4 = wl.C4
+    n = 3000
+    b = g.PhotonBatch(n, prec)
+    g.gray_init_rays_random(b, c4["a"], wl.R_OBS, c4["inc_deg"], c4["half_width"], c4["seed"])
+    y0, _, _ = gpu_state(b)
+    p = g.StepParams(rule=g.STEP_REL, frozen=True)
+    g.gray_integrate(b, max_steps=c4["peak_steps"], params=p)
+    y, st, ns = gpu_state(b)
+    cnt = g.gray_integrate_counters(b)
+    assert cnt["issued_steps"] >= n * c4["peak_steps"] and cnt["photon_steps"] == ns.sum()
+    # identical to the same photons run with normal termination (bitwise)
+    b2 = g.PhotonBatch(n, prec)
+    g.gray_init_rays_random(b2, c4["a"], wl.R_OBS, c4["inc_deg"], c4["half_width"], c4["seed"])
+    g.gray_integrate(b2, max_steps=c4["peak_steps"], params=g.StepParams(rule=g.STEP_REL))
+    assert torch.equal(b.x.view(torch.uint8), b2.x.view(torch.uint8)) and torch.equal(b.status, b2.status)
+    assert torch.equal(b.steps, b2.steps)
+    if prec == g.GRAY_F64:
+        ref = o.trace(c4["a"], wl.R_OBS, c4["inc_deg"], c4["half_width"], 0, 0, seed=c4["seed"], n=n, rule=o.STEP_REL,
+                      max_steps=c4["peak_steps"], threads=8)
+        same = (st == ref["status"]) & (ns == ref["steps"])
+        assert same.mean() > 0.995
+        fin = same & (st != g.BAD)
+        err = np.abs(y[fin] - ref["y"][fin]) / np.maximum(np.abs(ref["y"][fin]), 1.0)
+        assert np.quantile(err, 0.99) < 1e-9
+
+
+# ------------------------------------------------------------------------ classify / shadow
+@pytest.mark.parametrize("a,inc,W,n", [(0.9, 60.0, 10.0, 128), (0.0, 60.0, 10.0, 100)])
+def test_classify_and_shadow_edge_match_oracle_and_bardeen(a, inc, W, n):
+    out = g.trace_image(a, inc, W, n, n, params=g.StepParams(rule=g.STEP_EQ2), n_angles=360)
+    b = out["batch"]
+    _, st, _ = gpu_state(b)
+    cmap = out["capture_map"].cpu().numpy()
+    assert np.array_equal(cmap.ravel(), (st == g.CAPTURED).astype(np.uint8))      # bit-exact byte work
+    assert out["counts"] == [int((st == s).sum()) for s in range(4)]
+    ref, radius = o.shadow_stats(cmap, W, 360)
+    got = out["stats"]
+    assert got["n_captured"] == ref["n_captured"]
+    for k in ("area", "centroid_alpha", "centroid_beta", "alpha_min", "alpha_max", "D", "R_mean", "A"):
+        assert abs(got[k] - ref[k]) <= 1e-12 * max(1.0, abs(ref[k])), k
+    assert np.max(np.abs(out["radius"].cpu().numpy() - radius)) <= 1e-12
+    ex = cf.bardeen_stats(a, inc)
+    px = 2 * W / n
+    assert abs(got["area"] - ex["area"]) < 0.01 * ex["area"]
+    assert abs(got["D"] - ex["D"]) < px and abs(got["R_mean"] - ex["R_mean"]) < 0.5 * px
+
+
+# ------------------------------------------------------------------------------ edge cases
+def test_edge_cases_empty_single_partial_and_errors():
+    b = g.PhotonBatch(0)
+    g.gray_init_rays(b, 0.5, wl.R_OBS, 60.0, 10.0, 4, 4)
+    g.gray_integrate(b)
+    assert g.gray_classify(b) == [0, 0, 0, 0]
+    b = g.PhotonBatch(1, g.GRAY_F64)
+    g.gray_init_rays(b, 0.5, wl.R_OBS, 60.0, 10.0, 1, 1)     # the single pixel at (0, 0): a pole ray, any status
+    g.gray_integrate(b, max_steps=50)
+    assert int(b.steps.item()) == 50 or int(b.status.item()) != g.LIVE
+    # n_photons < n: the rest stays untouched
+    b = g.PhotonBatch(300)
+    g.gray_init_rays(b, 0.5, wl.R_OBS, 60.0, 10.0, 20, 15)
+    g.gray_integrate(b, n_photons=130)
+    _, st, n = gpu_state(b)
+    assert np.all(st[:130] != g.LIVE) and np.all(st[130:] == g.LIVE) and np.all(n[130:] == 0)
+    # max_steps = 0 is a no-op; a second call on finished photons is a no-op too
+    before = b.x.clone()
+    g.gray_integrate(b, n_photons=130)
+    assert torch.equal(before, b.x) and g.gray_integrate_counters(b)["photon_steps"] == 0
+    with pytest.raises(g.GrayError):
+        g.gray_integrate(b, n_photons=301)
+    with pytest.raises(g.GrayError):
+        g.gray_integrate(b, params=g.StepParams(h=-1.0))
+    with pytest.raises(g.GrayError):
+        g.gray_init_rays(b, 1.0, wl.R_OBS, 60.0, 10.0, 20, 15)
+    with pytest.raises(g.GrayError):
+        g.gray_init_rays(b, 0.5, wl.R_OBS, 60.0, 10.0, 10, 10)     # 300 photons do not fit a 10 x 10 image
+    g.gray_shadow_edge(b, 16)                                       # a full 20 x 15 grid: accepted
+    br = g.PhotonBatch(64)
+    g.gray_init_rays_random(br, 0.5, wl.R_OBS, 60.0, 10.0, 1)
+    with pytest.raises(g.GrayError):
+        g.gray_shadow_edge(br, 16)                                  # random pixels have no image grid
+
+
+def test_integrate_host_matches_device_path():
+    # the end-to-end entry point (host buffers, chunked, two streams) gives the device path's bits
+    a, inc, W, nx, ny = 0.9, 60.0, 10.0, 100, 77
+    n = nx * ny
+    for prec, dt in ((g.GRAY_F32, torch.float32), (g.GRAY_F64, torch.float64)):
+        b = g.PhotonBatch(n, prec)
+        g.gray_init_rays(b, a, wl.R_OBS, inc, W, nx, ny)
+        x_in, k_in = b.x.cpu().pin_memory(), b.k.cpu().pin_memory()
+        g.gray_integrate(b, params=g.StepParams(rule=g.STEP_EQ2))
+        cnt_dev = g.gray_integrate_counters(b)
+        x_out = torch.empty((n, 4), dtype=dt).pin_memory()
+        k_out = torch.empty((n, 4), dtype=dt).pin_memory()
+        status = torch.empty((n,), dtype=torch.uint8).pin_memory()
+        steps = torch.empty((n,), dtype=torch.int32).pin_memory()
+        chunk = 1000       # 8 chunks, ragged tail of 700
+        scratch = torch.empty((g.gray_host_scratch_bytes(chunk, prec),), dtype=torch.uint8, device="cuda")
+        cnt = g.gray_integrate_host(x_in, k_in, x_out, k_out, status, steps, a, wl.R_OBS, params=g.StepParams(rule=g.STEP_EQ2),
+                                    chunk=chunk, scratch=scratch)
+        assert torch.equal(x_out.view(torch.uint8), b.x.cpu().view(torch.uint8))
+        assert torch.equal(k_out.view(torch.uint8), b.k.cpu().view(torch.uint8))
+        assert torch.equal(status, b.status.cpu()) and torch.equal(steps, b.steps.cpu())
+        assert cnt["photon_steps"] == cnt_dev["photon_steps"] and cnt["photons_done"] == n
