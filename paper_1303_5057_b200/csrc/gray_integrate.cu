@@ -33,19 +33,27 @@ template <typename T> struct Tune;
 template <> struct Tune<float> { static constexpr int min_blocks = 4; };    // <= 128 registers/thread
 template <> struct Tune<double> { static constexpr int min_blocks = 2; };   // <= 255 registers/thread
 
+// HBM -> registers: (t, r, theta, phi), k^mu -> the kernel's variables (gray_math.cuh): d = r - r_+ and
+// theta folded into [0, pi/2].
 template <typename T>
-__device__ __forceinline__ void load_photon(const IntegrateArgs<T>& A, unsigned long long p, T y[8]) {
+__device__ __forceinline__ void load_photon(const IntegrateArgs<T>& A, unsigned long long p, T y[8], int& mirrored) {
   const typename Vec4T<T>::type xv = A.x[p], kv = A.k[p];
-  y[0] = xv.x; y[1] = xv.y; y[2] = xv.z; y[3] = xv.w;
+  y[0] = xv.x; y[1] = xv.y - A.K.rp; y[2] = xv.z; y[3] = xv.w;
   y[4] = kv.x; y[5] = kv.y; y[6] = kv.z; y[7] = kv.w;
+  mirrored = 0;
+  if (y[2] > T(1.57079632679489661923)) {
+    y[2] = pi_minus(y[2]);
+    y[6] = -y[6];
+    mirrored = 1;
+  }
 }
 
 template <typename T>
 __device__ __forceinline__ void store_photon(const IntegrateArgs<T>& A, unsigned long long p, const T y[8],
-                                             int st, uint32_t nst) {
+                                             int mirrored, int st, uint32_t nst) {
   typename Vec4T<T>::type xv, kv;
-  xv.x = y[0]; xv.y = y[1]; xv.z = y[2]; xv.w = y[3];
-  kv.x = y[4]; kv.y = y[5]; kv.z = y[6]; kv.w = y[7];
+  xv.x = y[0]; xv.y = y[1] + A.K.rp; xv.z = mirrored ? pi_minus(y[2]) : y[2]; xv.w = y[3];
+  kv.x = y[4]; kv.y = y[5]; kv.z = mirrored ? -y[6] : y[6]; kv.w = y[7];
   A.x[p] = xv;
   A.k[p] = kv;
   A.status[p] = (uint8_t)st;
@@ -65,7 +73,8 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<T> A) {
   const int lane = threadIdx.x & 31;
   const KerrConst<T> K = A.K;
 
-  T y[8];
+  T y[8], comp[8];
+  int mirrored = 0;
   unsigned long long idx = 0;
   uint32_t nst = 0, nst0 = 0, iss = 0;
   int fstat = GRAY_LIVE;
@@ -80,14 +89,16 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<T> A) {
     const uint32_t s = A.steps[p];
     if (st != GRAY_LIVE) return;
     if (s >= A.max_steps) { ++c_live; return; }
-    load_photon(A, p, y);
+    load_photon(A, p, y, mirrored);
+#pragma unroll
+    for (int i = 0; i < 8; ++i) comp[i] = T(0);
     idx = p;
     nst = nst0 = iss = s;
     fstat = GRAY_LIVE;
     have = true;
   };
   auto retire = [&](int st) {
-    store_photon(A, idx, y, st, nst);
+    store_photon(A, idx, y, mirrored, st, nst);
     c_steps += nst - nst0;
     if (st == GRAY_LIVE) ++c_live; else ++c_done;
     have = false;
@@ -121,30 +132,31 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<T> A) {
       if (have) {
         const T dl = step_size<T, RULE>(K, y);
         if (!FROZEN) {
-          rk4_step(K, y, dl);
-          remap_theta(y);
+          rk4_step(K, y, comp, dl);
+          remap_theta(y, comp, mirrored);
           ++nst;
           const int st = state_status(K, y);
           if (st != GRAY_LIVE || nst == A.max_steps) retire(st);
         } else {
-          T z[8];
+          T z[8], zc[8];
+          int zm = mirrored;
 #pragma unroll
-          for (int i = 0; i < 8; ++i) z[i] = y[i];
-          rk4_step(K, z, dl);
-          remap_theta(z);
+          for (int i = 0; i < 8; ++i) { z[i] = y[i]; zc[i] = comp[i]; }
+          rk4_step(K, z, zc, dl);
+          remap_theta(z, zc, zm);
           const int st = state_status(K, z);
           const bool adv = (fstat == GRAY_LIVE);
 #pragma unroll
-          for (int i = 0; i < 8; ++i) y[i] = adv ? z[i] : y[i];
+          for (int i = 0; i < 8; ++i) { y[i] = adv ? z[i] : y[i]; comp[i] = adv ? zc[i] : comp[i]; }
+          mirrored = adv ? zm : mirrored;
           nst += adv ? 1u : 0u;
           fstat = adv ? st : fstat;
           ++iss;
           if (iss == A.max_steps) retire(fstat);
         }
       }
-      ++c_iter;
-      if (!__any_sync(FULL, have)) break;
     }
+    c_iter += A.refill_interval;
   }
 
   c_steps = warp_sum(c_steps);
@@ -203,7 +215,7 @@ static int integrate(const gray_state* st, uint64_t n, uint32_t max_steps, const
   A.K.a = (T)a;
   A.K.a2 = (T)(a * a);
   A.K.rp = (T)rh;
-  A.K.rm = (T)(1.0 - root);
+  A.K.rpm = (T)(2.0 * root);
   A.K.h = (T)p->h;
   A.K.r_cap = (T)(p->r_capture_factor > 0.0 ? p->r_capture_factor * rh : rh + p->horizon_delta);
   A.K.r_esc = (T)(p->r_escape_factor * st->r_obs);

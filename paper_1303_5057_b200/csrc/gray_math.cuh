@@ -17,6 +17,13 @@
 //   dk^th /dl = 1/Sigma [ s c (2 r w^2/Sigma^2 + Delta (k^phi)^2 + a^2 ((k^th)^2 - (k^r)^2/Delta))
 //                         - 2 r k^r k^th ]
 // One sincos and three reciprocals (1/Sigma, 1/Delta, 1/s) per evaluation.
+//
+// Conditioning: inside the kernel the radial variable is the
+// height above the horizon  d = r - r_+  (so Delta = d (d + r_+ - r_-) keeps full relative
+// precision where the equations are singular), and the polar angle is kept in [0, pi/2] by the
+// reflection symmetry theta -> pi - theta, k^theta -> -k^theta of the Kerr metric (so the
+// absolute rounding of theta shrinks towards either pole, where the equations are singular
+// too).  Both are exact changes of variable of the same ODE; they are undone on store.
 #pragma once
 #include <cuda_runtime.h>
 #include <math.h>
@@ -33,43 +40,78 @@ namespace gray {
 template <typename T>
 struct KerrConst {
   T a, a2;        // spin and its square
-  T rp, rm;       // r_+ = 1 + sqrt(1 - a^2) (the horizon r_bh) and r_- = 1 - sqrt(1 - a^2)
+  T rp;           // r_+ = 1 + sqrt(1 - a^2): the horizon r_bh of P:75
+  T rpm;          // r_+ - r_- = 2 sqrt(1 - a^2)
   T h;            // step parameter (paper's Delta)
   T r_cap, r_esc; // termination radii
 };
 
+// Photon state as the kernel carries it: y = (t, d, th, phi, k^t, k^r, k^th, k^phi) with d = r - r_+ and
+// th in [0, pi/2]; `mirrored` says that the true polar angle is pi - th (and the true k^theta is -k^th).
+template <typename T>
+struct Photon {
+  T y[8];
+  int mirrored;
+};
+
 // ---- scalar helpers -------------------------------------------------------------------------
+// Reciprocal.  float: MUFU.RCP (relative error <= 1 ulp, B300_MICROARCH "XU"); its three uses per
+// right-hand side sit among ~80 roundings of half an ulp each, so it is not refined.
 GRAY_DEV float rcp(float x) {
 #if defined(__CUDA_ARCH__)
   float y;
-  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));   // MUFU.RCP, ~1 ulp
-  float e = fmaf(-x, y, 1.0f);                             // one Newton step -> < 1 ulp
-  return fmaf(y, e, y);
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
 #else
   return 1.0f / x;
 #endif
 }
 GRAY_DEV double rcp(double x) { return 1.0 / x; }
 
-GRAY_DEV void sincos_t(float x, float* s, float* c) { sincosf(x, s, c); }
+// sin and cos of x for |x| < ~100 (the kernel's theta stays within a step of [0, pi/2]).
+// float: quadrant j = rint(x 2/pi) by the add-magic-constant trick, r = x - j pi/2 with pi/2 split in
+// two floats (exact enough for small |j|), then near-minimax polynomials on [-pi/4, pi/4] fitted for
+// this kernel (max error 0.86 ulp for both, checked against fp64 over 2e6 points); no slow path, no
+// int<->float conversions (those run on the quarter-rate XU pipe).
+GRAY_DEV void sincos_t(float x, float* s, float* c) {
+#if defined(__CUDA_ARCH__)
+  const float q = fmaf(x, 0.636619772f, 12582912.0f);      // 1.5 * 2^23: the low mantissa bits of q hold j
+  const int j = __float_as_int(q);
+  const float jf = q - 12582912.0f;
+  float r = fmaf(jf, -1.57079637050628662109375f, x);      // float(pi/2)
+  r = fmaf(jf, 4.371139000186241e-08f, r);                 // pi/2 - float(pi/2)
+  const float u = r * r;
+  const float sp = fmaf(fmaf(-1.957778732e-04f, u, 8.332700469e-03f), u, -1.666666418e-01f);
+  const float sn = fmaf(r * u, sp, r);
+  const float cp = fmaf(fmaf(fmaf(2.445036807e-05f, u, -1.388748409e-03f), u, 4.166664928e-02f), u, -0.5f);
+  const float cs = fmaf(u, cp, 1.0f);
+  const bool swap = (j & 1) != 0;
+  const float ss = swap ? cs : sn, cc = swap ? sn : cs;
+  *s = __int_as_float(__float_as_int(ss) ^ ((j & 2) << 30));          // quadrants 2, 3: sin < 0
+  *c = __int_as_float(__float_as_int(cc) ^ (((j + 1) & 2) << 30));    // quadrants 1, 2: cos < 0
+#else
+  *s = sinf(x); *c = cosf(x);
+#endif
+}
 GRAY_DEV void sincos_t(double x, double* s, double* c) { sincos(x, s, c); }
 GRAY_DEV float abs_t(float x) { return fabsf(x); }
 GRAY_DEV double abs_t(double x) { return fabs(x); }
 GRAY_DEV float min_t(float x, float y) { return fminf(x, y); }
 GRAY_DEV double min_t(double x, double y) { return fmin(x, y); }
 
-// ---- right-hand side: accelerations dk^mu/dlambda at (r, th) for momentum (kt, kr, kh, kp) ------
+// ---- right-hand side: accelerations dk^mu/dlambda at (d = r - r_+, th) for momentum (kt, kr, kh, kp) ----
 template <typename T>
-GRAY_DEV void geodesic_accel(const KerrConst<T>& K, T r, T th, T kt, T kr, T kh, T kp,
+GRAY_DEV void geodesic_accel(const KerrConst<T>& K, T d, T th, T kt, T kr, T kh, T kp,
                              T& at, T& ar, T& ah, T& ap) {
   T s, c;
   sincos_t(th, &s, &c);
+  const T r = d + K.rp;
   const T r2 = r * r, c2 = c * c, s2 = s * s, sc = s * c;
   const T a2c2 = K.a2 * c2;
   const T Sg = r2 + a2c2;                       // Sigma
   const T P = r2 - a2c2;
   const T rho = r2 + K.a2;
-  const T Dl = (r - K.rp) * (r - K.rm);         // Delta, product form: no cancellation at the horizon
+  const T Dl = d * (d + K.rpm);                 // Delta = (r - r_+)(r - r_-): no cancellation at the horizon
   const T iS = rcp(Sg), iD = rcp(Dl), is = rcp(s);
   const T cot = c * is;
   const T iS2 = iS * iS;
@@ -95,18 +137,28 @@ GRAY_DEV void geodesic_accel(const KerrConst<T>& K, T r, T th, T kt, T kr, T kh,
 }
 
 // ---- step size (gray.h gray_step_rule; paper eq. (2)) -----------------------------------------
+// y[1] = d = r - r_+.  float: the two quotients of eq. (2) are formed with MUFU.RCP (1 ulp): the step
+// size is a free parameter of the scheme, an ulp of it is far below the truncation error it controls.
 template <typename T, int RULE>
 GRAY_DEV T step_size(const KerrConst<T>& K, const T y[8]) {
-  if (RULE == 0) return -K.h * y[1];
+  const T r = y[1] + K.rp;
+  if (RULE == 0) return -K.h * r;
   const T akr = abs_t(y[5]);
-  const T d1 = K.h / (akr / y[1] + abs_t(y[6]) + abs_t(y[7]));
-  const T d2 = (y[1] - K.rp) / (T(2) * akr);
+  if (sizeof(T) == 4) {
+    const T d1 = K.h * r * rcp(akr + r * (abs_t(y[6]) + abs_t(y[7])));
+    const T d2 = T(0.5) * y[1] * rcp(akr);
+    return -min_t(d1, d2);
+  }
+  const T d1 = K.h / (akr / r + abs_t(y[6]) + abs_t(y[7]));
+  const T d2 = y[1] / (T(2) * akr);
   return -(d1 < d2 ? d1 : d2);
 }
 
-// ---- one classical RK4 step of y = (t, r, th, phi, k^t, k^r, k^th, k^phi) -------------------
+// ---- one classical RK4 step of y = (t, d, th, phi, k^t, k^r, k^th, k^phi) -------------------
+// `comp` carries, for the float build, the rounding error of each state update into the next one
+// (compensated summation): y + comp is the state to roughly twice the working precision.
 template <typename T>
-GRAY_DEV void rk4_step(const KerrConst<T>& K, T y[8], T dl) {
+GRAY_DEV void rk4_step(const KerrConst<T>& K, T y[8], T comp[8], T dl) {
   T acc[8], w[8], f[4];
   const T hdl = T(0.5) * dl;
   // stage 1
@@ -141,25 +193,52 @@ GRAY_DEV void rk4_step(const KerrConst<T>& K, T y[8], T dl) {
   // stage 4
   geodesic_accel(K, w[1], w[2], w[4], w[5], w[6], w[7], f[0], f[1], f[2], f[3]);
   const T dl6 = dl * T(1.0 / 6.0);
+  if (sizeof(T) == 4) {
 #pragma unroll
-  for (int i = 0; i < 4; ++i) {
-    y[i] += dl6 * (acc[i] + w[4 + i]);
-    y[4 + i] += dl6 * (acc[4 + i] + f[i]);
+    for (int i = 0; i < 8; ++i) {
+      const T inc = dl6 * (acc[i] + (i < 4 ? w[4 + i] : f[i - 4])) + comp[i];
+      const T s = y[i] + inc;
+      comp[i] = inc - (s - y[i]);          // Fast2Sum: exact whenever |y| >= |inc|
+      y[i] = s;
+    }
+  } else {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      y[i] += dl6 * (acc[i] + w[4 + i]);
+      y[4 + i] += dl6 * (acc[4 + i] + f[i]);
+    }
   }
 }
 
-// ---- theta remap, paper eq. (3), P:87 ---------------------------------------------------------------
+// pi and 2 pi minus x with pi split in two parts of the working precision
+GRAY_DEV float pi_minus(float x) { return (3.14159274101257324219f - x) - 8.742278000372485e-08f; }
+GRAY_DEV double pi_minus(double x) { return (3.141592653589793116 - x) + 1.2246467991473532e-16; }
+GRAY_DEV float two_pi_minus(float x) { return (6.28318548202514648438f - x) - 1.748455600074497e-07f; }
+GRAY_DEV double two_pi_minus(double x) { return (6.283185307179586232 - x) + 2.4492935982947064e-16; }
+
+// ---- theta remap, paper eq. (3), followed by the reflection that keeps th in [0, pi/2] ----------
+// Eq. (3) acts on the true polar angle.  For a mirrored photon (true angle pi - th) the true angle
+// exceeds pi when th < 0 and is negative when th > pi, so the sign of the phi shift flips with it.
 template <typename T>
-GRAY_DEV void remap_theta(T y[8]) {
+GRAY_DEV void remap_theta(T y[8], T comp[8], int& mirrored) {
   const T pi = T(3.14159265358979323846);
+  const T shift = mirrored ? -pi : pi;
   if (y[2] > pi) {
-    y[2] = T(2) * pi - y[2];
-    y[3] += pi;
+    y[2] = two_pi_minus(y[2]);
+    y[3] += shift;
     y[6] = -y[6];
+    comp[2] = -comp[2]; comp[6] = -comp[6];
   } else if (y[2] < T(0)) {
     y[2] = -y[2];
-    y[3] -= pi;
+    y[3] -= shift;
     y[6] = -y[6];
+    comp[2] = -comp[2]; comp[6] = -comp[6];
+  }
+  if (y[2] > T(1.57079632679489661923)) {
+    y[2] = pi_minus(y[2]);
+    y[6] = -y[6];
+    comp[2] = -comp[2]; comp[6] = -comp[6];
+    mirrored ^= 1;
   }
 }
 
@@ -170,8 +249,9 @@ GRAY_DEV int state_status(const KerrConst<T>& K, const T y[8]) {
 #pragma unroll
   for (int i = 0; i < 8; ++i) z += T(0) * y[i];     // inf * 0 = NaN, NaN * 0 = NaN, finite * 0 = 0
   if (!(z == T(0))) return 3;
-  if (y[1] < K.r_cap) return 1;
-  if (y[1] > K.r_esc) return 2;
+  const T r = y[1] + K.rp;
+  if (r < K.r_cap) return 1;
+  if (r > K.r_esc) return 2;
   return 0;
 }
 

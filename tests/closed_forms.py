@@ -99,6 +99,15 @@ def captured_exact(a, xi, eta):
     return not np.any(real > horizon(a) * (1 + 1e-12))
 
 
+def sin_theta_min(a, xi, eta):
+    """Sine of the smallest polar angle a photon with (xi, eta), eta >= 0, can reach: the root of
+    Theta(theta) = eta + a^2 cos^2(theta) - xi^2 cot^2(theta) = 0.  With u = cos^2(theta):
+    a^2 u^2 + (eta + xi^2 - a^2) u - eta = 0, u_max its non-negative root."""
+    B = eta + xi * xi - a * a
+    u = 2.0 * eta / (B + np.sqrt(B * B + 4.0 * a * a * eta))
+    return np.sqrt(np.clip(1.0 - u, 0.0, 1.0))
+
+
 def schwarzschild_dphi(b, r_start, r_end):
     """|change of phi| of a Schwarzschild (M = 1) photon of impact parameter b > sqrt(27) that
     comes in from r_start, turns at r_min and goes out to r_end (textbook orbit integral,

@@ -42,3 +42,23 @@ def rel_err_final(y_gpu, y_ref):
     d = np.abs(y_gpu[:, 1:4] - y_ref[:, 1:4])
     den = np.stack([np.abs(y_ref[:, 1]), np.maximum(np.abs(y_ref[:, 2]), 1e-2), np.maximum(np.abs(y_ref[:, 3]), 1.0)], 1)
     return (d / den).max(axis=1)
+
+
+def xi_eta_of(a, y0):
+    """(xi, eta) = (L_z / E, Q / E^2) of initial states, from the oracle's invariants."""
+    inv = np.array([o.invariants(a, v) for v in y0])
+    return inv[:, 1] / inv[:, 0], inv[:, 2] / inv[:, 0] ** 2
+
+
+def exact_capture(a, xi, eta):
+    return np.array([cf.captured_exact(a, x, e) for x, e in zip(xi, eta)])
+
+
+POLE_SIN = 0.05
+
+
+def pole_band(a, xi, eta):
+    """Rays whose polar turning point lies within asin(POLE_SIN) ~ 2.9 deg of the spin axis (DESIGN.md reading
+    R14): Boyer-Lindquist coordinates are singular there and an absolute rounding error in theta becomes a
+    relative error delta/theta in k^phi; the paper treats this band separately."""
+    return cf.sin_theta_min(a, xi, np.maximum(eta, 0.0)) < POLE_SIN
