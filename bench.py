@@ -47,6 +47,7 @@ def parse():
     ap.add_argument("--case", default="realistic", choices=["realistic", "peak"])
     ap.add_argument("--schedule", default="refill", choices=["refill", "static"])
     ap.add_argument("--refill-interval", type=int, default=0)
+    ap.add_argument("--photons-per-thread", type=int, default=0, help="0 = library default (2 for f32: packed FFMA2), 1, 2")
     ap.add_argument("--e2e-log2n", type=int, default=-1, help="photons per GPU of the host-buffer run (default min(log2n, 26))")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -178,7 +179,8 @@ def run_gray(args):
     max_steps = c4["peak_steps"] if peak_case else wl.MAX_STEPS
     params = g.StepParams(h=wl.H, r_capture_factor=wl.R_CAPTURE_FACTOR, r_escape_factor=wl.R_ESCAPE_FACTOR, rule=rule,
                           schedule=g.SCHED_REFILL if args.schedule == "refill" else g.SCHED_STATIC,
-                          refill_interval=args.refill_interval, frozen=peak_case)
+                          refill_interval=args.refill_interval, frozen=peak_case,
+                          photons_per_thread=args.photons_per_thread)
     batch = g.PhotonBatch(n, prec, device=dev)
     p0 = rank * n                                   # weak scaling: every rank its own photon range
 

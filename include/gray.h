@@ -120,6 +120,11 @@ typedef struct {
                                 live photon is stepped until its counter reaches max_steps with no
                                 early exit; once a test fires its state, status and step count are
                                 frozen by select while the arithmetic continues                      */
+  int32_t photons_per_thread; /* 0 = default (2 for GRAY_F32, 1 for GRAY_F64); 2 = two photons per thread
+                                advanced together by the packed sm_100a FP32 instructions (FFMA2 /
+                                FMUL2 / FADD2, GRAY_F32 only); 1 = one photon per thread, scalar
+                                instructions.  Per-photon results are bit-identical for 1 and 2.       */
+  int32_t reserved;          /* must be 0                                                             */
 } gray_step_params;
 
 /* Bytes of device workspace gray_integrate / gray_classify / gray_shadow_edge need (queue head and

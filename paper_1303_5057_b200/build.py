@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgray.so")
 SOURCES = ["gray_api.cu", "gray_init.cu", "gray_integrate.cu", "gray_shadow.cu", "gray_host.cu"]
-HEADERS = [os.path.join(CSRC, "gray_internal.h"), os.path.join(CSRC, "gray_math.cuh"),
+HEADERS = [os.path.join(CSRC, "gray_internal.h"), os.path.join(CSRC, "gray_math.cuh"), os.path.join(CSRC, "gray_vec.cuh"),
            os.path.join(os.path.dirname(HERE), "include", "gray.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]

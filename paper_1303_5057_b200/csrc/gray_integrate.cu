@@ -1,64 +1,40 @@
 // gray_integrate.cu — the integrator kernel of libgray and gray_integrate() (include/gray.h).
 //
-// One photon per thread, its 8-component state in registers from the moment it is loaded until it
-// terminates ("GRay integrates each geodesic for many steps in a single data load", P:81 fn 5).
-// What differs from the paper's fixed grid of 64-thread blocks: the kernel is persistent
-// (148 SMs x resident blocks) and a lane whose photon has terminated is refilled from a device-side
-// queue, so a warp never idles on its slowest ray; HBM is touched once per photon on load and once
-// on retirement, with 16-byte vector accesses.
+// One photon per lane of a vector type V (gray_vec.cuh): float / double = one photon per thread, f2 = two
+// fp32 photons per thread in packed FFMA2 / FMUL2 / FADD2 instructions.  A photon's 8-component state
+// stays in registers from the moment it is loaded until it terminates ("GRay integrates each geodesic
+// for many steps in a single data load", P:81 fn 5).  What differs from the paper's fixed grid of
+// 64-thread blocks: the kernel is persistent (148 SMs x resident blocks) and a lane whose
+// photon has terminated is refilled from a device-side queue, so a warp never idles on its slowest
+// ray; HBM is touched once per photon on load and once on retirement, with 16-byte vector accesses.
 #include "gray_internal.h"
 #include "gray_math.cuh"
 
 namespace gray {
 
-template <typename T> struct Vec4T;
+template <typename S> struct Vec4T;
 template <> struct Vec4T<float> { using type = float4; };
 template <> struct Vec4T<double> { using type = double4; };
 
-template <typename T>
+template <typename V>
 struct IntegrateArgs {
-  typename Vec4T<T>::type* x;
-  typename Vec4T<T>::type* k;
+  using S = typename VT<V>::S;
+  typename Vec4T<S>::type* x;
+  typename Vec4T<S>::type* k;
   uint8_t* status;
   uint32_t* steps;
   unsigned long long n;
   uint32_t max_steps;
   int refill_interval;
-  KerrConst<T> K;
   Workspace* ws;
+  Consts<V> K;
 };
 
 constexpr int kBlock = 128;
-template <typename T> struct Tune;
+template <typename V> struct Tune;
 template <> struct Tune<float> { static constexpr int min_blocks = 4; };    // <= 128 registers/thread
+template <> struct Tune<f2> { static constexpr int min_blocks = 4; };       // <= 128 registers/thread
 template <> struct Tune<double> { static constexpr int min_blocks = 2; };   // <= 255 registers/thread
-
-// HBM -> registers: (t, r, theta, phi), k^mu -> the kernel's variables (gray_math.cuh): d = r - r_+ and
-// theta folded into [0, pi/2].
-template <typename T>
-__device__ __forceinline__ void load_photon(const IntegrateArgs<T>& A, unsigned long long p, T y[8], int& mirrored) {
-  const typename Vec4T<T>::type xv = A.x[p], kv = A.k[p];
-  y[0] = xv.x; y[1] = xv.y - A.K.rp; y[2] = xv.z; y[3] = xv.w;
-  y[4] = kv.x; y[5] = kv.y; y[6] = kv.z; y[7] = kv.w;
-  mirrored = 0;
-  if (y[2] > T(1.57079632679489661923)) {
-    y[2] = pi_minus(y[2]);
-    y[6] = -y[6];
-    mirrored = 1;
-  }
-}
-
-template <typename T>
-__device__ __forceinline__ void store_photon(const IntegrateArgs<T>& A, unsigned long long p, const T y[8],
-                                             int mirrored, int st, uint32_t nst) {
-  typename Vec4T<T>::type xv, kv;
-  xv.x = y[0]; xv.y = y[1] + A.K.rp; xv.z = mirrored ? pi_minus(y[2]) : y[2]; xv.w = y[3];
-  kv.x = y[4]; kv.y = y[5]; kv.z = mirrored ? -y[6] : y[6]; kv.w = y[7];
-  A.x[p] = xv;
-  A.k[p] = kv;
-  A.status[p] = (uint8_t)st;
-  A.steps[p] = nst;
-}
 
 __device__ __forceinline__ unsigned long long warp_sum(unsigned long long v) {
 #pragma unroll
@@ -66,93 +42,152 @@ __device__ __forceinline__ unsigned long long warp_sum(unsigned long long v) {
   return v;
 }
 
-template <typename T, int RULE, int SCHED, bool FROZEN>
-__global__ void __launch_bounds__(kBlock, Tune<T>::min_blocks)
-integrate_kernel(const __grid_constant__ IntegrateArgs<T> A) {
+template <typename V, int RULE, int SCHED, bool FROZEN>
+__global__ void __launch_bounds__(kBlock, Tune<V>::min_blocks)
+integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
+  using S = typename VT<V>::S;
+  constexpr int N = VT<V>::N;
   constexpr unsigned FULL = 0xffffffffu;
   const int lane = threadIdx.x & 31;
-  const KerrConst<T> K = A.K;
+  const Consts<V>& K = A.K;
 
-  T y[8], comp[8];
-  int mirrored = 0;
-  unsigned long long idx = 0;
-  uint32_t nst = 0, nst0 = 0, iss = 0;
-  int fstat = GRAY_LIVE;
-  bool have = false;
+  V y[8], comp[8];
+  int mirrored[N];
+  unsigned long long idx[N];
+  uint32_t nst[N], nst0[N], iss[N];
+  int fstat[N];
+  bool have[N];
   bool exhausted = (SCHED == GRAY_SCHED_STATIC);
   unsigned long long c_steps = 0;
   unsigned int c_done = 0, c_live = 0, c_iter = 0;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) { y[i] = K.one; comp[i] = K.zero; }
+#pragma unroll
+  for (int l = 0; l < N; ++l) { have[l] = false; mirrored[l] = 0; idx[l] = 0; nst[l] = nst0[l] = iss[l] = 0; fstat[l] = GRAY_LIVE; }
 
-  // take photon p if it is live and has steps left
-  auto take = [&](unsigned long long p) {
+  // HBM -> registers: photon p into slot l, if it is live and has steps left.  (t, r, theta, phi), k^mu ->
+  // the kernel's variables (gray_math.cuh): d = r - r_+ and theta folded into [0, pi/2].
+  auto take = [&](int l, unsigned long long p) {
     const uint8_t st = A.status[p];
     const uint32_t s = A.steps[p];
     if (st != GRAY_LIVE) return;
     if (s >= A.max_steps) { ++c_live; return; }
-    load_photon(A, p, y, mirrored);
+    const typename Vec4T<S>::type xv = A.x[p], kv = A.k[p];
+    S th = xv.z, kh = kv.z;
+    int m = 0;
+    if (th > S(1.57079632679489661923)) { th = pi_minus(th); kh = sneg(kh); m = 1; }
+    vset(y[0], l, xv.x); vset(y[1], l, xv.y - vget(K.rp, 0)); vset(y[2], l, th); vset(y[3], l, xv.w);
+    vset(y[4], l, kv.x); vset(y[5], l, kv.y); vset(y[6], l, kh); vset(y[7], l, kv.w);
 #pragma unroll
-    for (int i = 0; i < 8; ++i) comp[i] = T(0);
-    idx = p;
-    nst = nst0 = iss = s;
-    fstat = GRAY_LIVE;
-    have = true;
+    for (int i = 0; i < 8; ++i) vset(comp[i], l, S(0));
+    mirrored[l] = m;
+    idx[l] = p;
+    nst[l] = nst0[l] = iss[l] = s;
+    fstat[l] = GRAY_LIVE;
+    have[l] = true;
   };
-  auto retire = [&](int st) {
-    store_photon(A, idx, y, mirrored, st, nst);
-    c_steps += nst - nst0;
+  // registers -> HBM
+  auto retire = [&](int l, int st) {
+    typename Vec4T<S>::type xv, kv;
+    const S th = vget(y[2], l), kh = vget(y[6], l);
+    xv.x = vget(y[0], l); xv.y = vget(y[1], l) + vget(K.rp, 0); xv.z = mirrored[l] ? pi_minus(th) : th; xv.w = vget(y[3], l);
+    kv.x = vget(y[4], l); kv.y = vget(y[5], l); kv.z = mirrored[l] ? sneg(kh) : kh; kv.w = vget(y[7], l);
+    const unsigned long long p = idx[l];
+    A.x[p] = xv;
+    A.k[p] = kv;
+    A.status[p] = (uint8_t)st;
+    A.steps[p] = nst[l];
+    c_steps += nst[l] - nst0[l];
     if (st == GRAY_LIVE) ++c_live; else ++c_done;
-    have = false;
+    have[l] = false;
   };
 
   if (SCHED == GRAY_SCHED_STATIC) {
-    const unsigned long long p = (unsigned long long)blockIdx.x * kBlock + threadIdx.x;
-    if (p < A.n) take(p);
+#pragma unroll
+    for (int l = 0; l < N; ++l) {
+      const unsigned long long p = ((unsigned long long)blockIdx.x * N + l) * kBlock + threadIdx.x;
+      if (p < A.n) take(l, p);
+    }
   }
 
   for (;;) {
     if (SCHED == GRAY_SCHED_REFILL && !exhausted) {
-      const unsigned need = __ballot_sync(FULL, !have);
-      if (need) {
-        const int cnt = __popc(need), leader = __ffs(need) - 1;
+      unsigned need[N];
+      int cnt = 0;
+#pragma unroll
+      for (int l = 0; l < N; ++l) { need[l] = __ballot_sync(FULL, !have[l]); cnt += __popc(need[l]); }
+      if (cnt) {
         unsigned long long base = 0;
-        if (lane == leader) base = atomicAdd(&A.ws->queue_head, (unsigned long long)cnt);
-        base = __shfl_sync(FULL, base, leader);
-        if (!have) {
-          const unsigned long long p = base + __popc(need & ((1u << lane) - 1u));
-          if (p < A.n) take(p);
+        if (lane == 0) base = atomicAdd(&A.ws->queue_head, (unsigned long long)cnt);
+        base = __shfl_sync(FULL, base, 0);
+        int off = 0;
+#pragma unroll
+        for (int l = 0; l < N; ++l) {
+          if (!have[l]) {
+            const unsigned long long p = base + off + __popc(need[l] & ((1u << lane) - 1u));
+            if (p < A.n) take(l, p);
+          }
+          off += __popc(need[l]);
         }
         if (base + cnt >= A.n) exhausted = true;
       }
     }
-    if (!__any_sync(FULL, have)) {
+    bool any = false;
+#pragma unroll
+    for (int l = 0; l < N; ++l) any |= have[l];
+    if (!__any_sync(FULL, any)) {
       if (exhausted) break;
       continue;
     }
     for (int it = 0; it < A.refill_interval; ++it) {
-      if (have) {
-        const T dl = step_size<T, RULE>(K, y);
+      any = false;
+#pragma unroll
+      for (int l = 0; l < N; ++l) any |= have[l];
+      if (any) {
+        const V dl = step_size<V, RULE>(K, y[1], y[5], y[6], y[7]);
         if (!FROZEN) {
           rk4_step(K, y, comp, dl);
-          remap_theta(y, comp, mirrored);
-          ++nst;
-          const int st = state_status(K, y);
-          if (st != GRAY_LIVE || nst == A.max_steps) retire(st);
+          const V z = nonfinite_probe(K, y);
+          const V r = vadd(y[1], K.rp);
+#pragma unroll
+          for (int l = 0; l < N; ++l) {
+            if (have[l]) {
+              S th = vget(y[2], l), ph = vget(y[3], l), kh = vget(y[6], l), c2 = vget(comp[2], l), c6 = vget(comp[6], l);
+              remap_theta(th, ph, kh, c2, c6, mirrored[l]);
+              vset(y[2], l, th); vset(y[3], l, ph); vset(y[6], l, kh); vset(comp[2], l, c2); vset(comp[6], l, c6);
+              ++nst[l];
+              const int st = state_status(vget(z, l), vget(r, l), K.r_cap, K.r_esc);
+              if (st != GRAY_LIVE || nst[l] == A.max_steps) retire(l, st);
+            }
+          }
         } else {
-          T z[8], zc[8];
-          int zm = mirrored;
+          V w[8], wc[8];
 #pragma unroll
-          for (int i = 0; i < 8; ++i) { z[i] = y[i]; zc[i] = comp[i]; }
-          rk4_step(K, z, zc, dl);
-          remap_theta(z, zc, zm);
-          const int st = state_status(K, z);
-          const bool adv = (fstat == GRAY_LIVE);
+          for (int i = 0; i < 8; ++i) { w[i] = y[i]; wc[i] = comp[i]; }
+          rk4_step(K, w, wc, dl);
+          const V z = nonfinite_probe(K, w);
+          const V r = vadd(w[1], K.rp);
 #pragma unroll
-          for (int i = 0; i < 8; ++i) { y[i] = adv ? z[i] : y[i]; comp[i] = adv ? zc[i] : comp[i]; }
-          mirrored = adv ? zm : mirrored;
-          nst += adv ? 1u : 0u;
-          fstat = adv ? st : fstat;
-          ++iss;
-          if (iss == A.max_steps) retire(fstat);
+          for (int l = 0; l < N; ++l) {
+            if (have[l]) {
+              S th = vget(w[2], l), ph = vget(w[3], l), kh = vget(w[6], l), c2 = vget(wc[2], l), c6 = vget(wc[6], l);
+              int wm = mirrored[l];
+              remap_theta(th, ph, kh, c2, c6, wm);
+              vset(w[2], l, th); vset(w[3], l, ph); vset(w[6], l, kh); vset(wc[2], l, c2); vset(wc[6], l, c6);
+              const int st = state_status(vget(z, l), vget(r, l), K.r_cap, K.r_esc);
+              const bool adv = (fstat[l] == GRAY_LIVE);
+#pragma unroll
+              for (int i = 0; i < 8; ++i) {
+                vset(y[i], l, adv ? vget(w[i], l) : vget(y[i], l));
+                vset(comp[i], l, adv ? vget(wc[i], l) : vget(comp[i], l));
+              }
+              mirrored[l] = adv ? wm : mirrored[l];
+              nst[l] += adv ? 1u : 0u;
+              fstat[l] = adv ? st : fstat[l];
+              ++iss[l];
+              if (iss[l] == A.max_steps) retire(l, fstat[l]);
+            }
+          }
         }
       }
     }
@@ -164,16 +199,17 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<T> A) {
   const unsigned long long live = warp_sum((unsigned long long)c_live);
   if (lane == 0) {
     if (c_steps) atomicAdd(&A.ws->photon_steps, c_steps);
-    if (c_iter) atomicAdd(&A.ws->issued_steps, 32ull * c_iter);
+    if (c_iter) atomicAdd(&A.ws->issued_steps, (unsigned long long)(32 * N) * c_iter);
     if (done) atomicAdd(&A.ws->photons_done, done);
     if (live) atomicAdd(&A.ws->photons_live, live);
   }
 }
 
-template <typename T, int RULE, int SCHED, bool FROZEN>
-static int launch(const IntegrateArgs<T>& A, cudaStream_t stream) {
-  auto kern = integrate_kernel<T, RULE, SCHED, FROZEN>;
-  unsigned long long blocks_needed = (A.n + kBlock - 1) / kBlock;
+template <typename V, int RULE, int SCHED, bool FROZEN>
+static int launch(const IntegrateArgs<V>& A, cudaStream_t stream) {
+  auto kern = integrate_kernel<V, RULE, SCHED, FROZEN>;
+  constexpr unsigned long long per_block = (unsigned long long)kBlock * VT<V>::N;
+  unsigned long long blocks_needed = (A.n + per_block - 1) / per_block;
   unsigned int grid;
   if (SCHED == GRAY_SCHED_STATIC) {
     if (blocks_needed > 0x7fffffffull) { set_error("n too large for the static schedule"); return GRAY_ERR_ARG; }
@@ -190,39 +226,35 @@ static int launch(const IntegrateArgs<T>& A, cudaStream_t stream) {
   return GRAY_OK;
 }
 
-template <typename T, int RULE, int SCHED>
-static int dispatch_frozen(const IntegrateArgs<T>& A, bool frozen, cudaStream_t s) {
-  return frozen ? launch<T, RULE, SCHED, true>(A, s) : launch<T, RULE, SCHED, false>(A, s);
+template <typename V, int RULE, int SCHED>
+static int dispatch_frozen(const IntegrateArgs<V>& A, bool frozen, cudaStream_t s) {
+  return frozen ? launch<V, RULE, SCHED, true>(A, s) : launch<V, RULE, SCHED, false>(A, s);
 }
-template <typename T, int RULE>
-static int dispatch_sched(const IntegrateArgs<T>& A, int sched, bool frozen, cudaStream_t s) {
-  return sched == GRAY_SCHED_STATIC ? dispatch_frozen<T, RULE, GRAY_SCHED_STATIC>(A, frozen, s)
-                                    : dispatch_frozen<T, RULE, GRAY_SCHED_REFILL>(A, frozen, s);
+template <typename V, int RULE>
+static int dispatch_sched(const IntegrateArgs<V>& A, int sched, bool frozen, cudaStream_t s) {
+  return sched == GRAY_SCHED_STATIC ? dispatch_frozen<V, RULE, GRAY_SCHED_STATIC>(A, frozen, s)
+                                    : dispatch_frozen<V, RULE, GRAY_SCHED_REFILL>(A, frozen, s);
 }
 
-template <typename T>
+template <typename V>
 static int integrate(const gray_state* st, uint64_t n, uint32_t max_steps, const gray_step_params* p,
                      Workspace* ws, cudaStream_t stream) {
-  IntegrateArgs<T> A;
-  A.x = (typename Vec4T<T>::type*)st->x_dev;
-  A.k = (typename Vec4T<T>::type*)st->k_dev;
+  using S = typename VT<V>::S;
+  IntegrateArgs<V> A;
+  A.x = (typename Vec4T<S>::type*)st->x_dev;
+  A.k = (typename Vec4T<S>::type*)st->k_dev;
   A.status = st->status_dev;
   A.steps = st->steps_dev;
   A.n = n;
   A.max_steps = max_steps;
   A.refill_interval = p->refill_interval > 0 ? p->refill_interval : 8;
-  const double a = st->a, root = sqrt(1.0 - a * a), rh = 1.0 + root;
-  A.K.a = (T)a;
-  A.K.a2 = (T)(a * a);
-  A.K.rp = (T)rh;
-  A.K.rpm = (T)(2.0 * root);
-  A.K.h = (T)p->h;
-  A.K.r_cap = (T)(p->r_capture_factor > 0.0 ? p->r_capture_factor * rh : rh + p->horizon_delta);
-  A.K.r_esc = (T)(p->r_escape_factor * st->r_obs);
+  const double a = st->a, rh = 1.0 + sqrt(1.0 - a * a);
+  A.K = make_consts<V>(a, p->h, p->r_capture_factor > 0.0 ? p->r_capture_factor * rh : rh + p->horizon_delta,
+                       p->r_escape_factor * st->r_obs);
   A.ws = ws;
   const bool frozen = p->frozen != 0;
-  return p->rule == GRAY_STEP_EQ2 ? dispatch_sched<T, GRAY_STEP_EQ2>(A, p->schedule, frozen, stream)
-                                  : dispatch_sched<T, GRAY_STEP_REL>(A, p->schedule, frozen, stream);
+  return p->rule == GRAY_STEP_EQ2 ? dispatch_sched<V, GRAY_STEP_EQ2>(A, p->schedule, frozen, stream)
+                                  : dispatch_sched<V, GRAY_STEP_REL>(A, p->schedule, frozen, stream);
 }
 
 }  // namespace gray
@@ -239,6 +271,8 @@ int gray_integrate(gray_state* state, uint64_t n_photons, uint32_t max_steps, co
   if (params->rule != GRAY_STEP_REL && params->rule != GRAY_STEP_EQ2) { set_error("bad step rule %d", params->rule); return GRAY_ERR_ARG; }
   if (params->schedule != GRAY_SCHED_REFILL && params->schedule != GRAY_SCHED_STATIC) { set_error("bad schedule %d", params->schedule); return GRAY_ERR_ARG; }
   if (params->refill_interval < 0) { set_error("refill_interval must be >= 0"); return GRAY_ERR_ARG; }
+  if (params->photons_per_thread < 0 || params->photons_per_thread > 2) { set_error("photons_per_thread must be 0 (default), 1 or 2"); return GRAY_ERR_ARG; }
+  if (params->photons_per_thread == 2 && state->prec != GRAY_F32) { set_error("photons_per_thread = 2 (packed FP32 instructions) needs GRAY_F32"); return GRAY_ERR_UNSUPPORTED; }
   if (!(params->h > 0.0) || !(params->r_escape_factor > 0.0) || params->r_capture_factor < 0.0 ||
       (params->r_capture_factor == 0.0 && !(params->horizon_delta >= 0.0))) {
     set_error("step parameters out of domain (h > 0, r_escape_factor > 0, r_capture_factor >= 0, horizon_delta >= 0)");
@@ -250,8 +284,9 @@ int gray_integrate(gray_state* state, uint64_t n_photons, uint32_t max_steps, co
   Workspace* ws = (Workspace*)workspace_dev;
   GRAY_CUDA(cudaMemsetAsync(ws, 0, 256, stream));   // queue head and gray_counters
   if (n_photons == 0 || max_steps == 0) return GRAY_OK;
-  return state->prec == GRAY_F32 ? integrate<float>(state, n_photons, max_steps, params, ws, stream)
-                                 : integrate<double>(state, n_photons, max_steps, params, ws, stream);
+  if (state->prec == GRAY_F64) return integrate<double>(state, n_photons, max_steps, params, ws, stream);
+  return params->photons_per_thread == 1 ? integrate<float>(state, n_photons, max_steps, params, ws, stream)
+                                         : integrate<f2>(state, n_photons, max_steps, params, ws, stream);
 }
 
 int gray_integrate_counters(const void* workspace_dev, gray_counters* counters_host, void* cuda_stream) {

@@ -1,5 +1,6 @@
-// gray_math.cuh — per-photon arithmetic of the integrator: Kerr geodesic right-hand side, RK4
-// step, step rules, theta remap.  Templated on the scalar type (float / double builds).
+// gray_math.cuh — per-photon arithmetic of the integrator: Kerr geodesic right-hand side, RK4 step,
+// step rules, theta remap, termination tests.  Templated on the vector type V of gray_vec.cuh
+// (float, double, or f2 = two fp32 photons per thread in packed FFMA2 / FMUL2 / FADD2 instructions).
 //
 // The equations are the second-order geodesic equations of the Kerr metric in Boyer-Lindquist
 // coordinates (paper P:23; the 20 non-zero Christoffel symbols are listed in SURVEY.md
@@ -7,251 +8,261 @@
 //     Sigma = r^2 + a^2 cos^2(th),  Delta = (r - r_+)(r - r_-),  P = r^2 - a^2 cos^2(th),
 //     rho = r^2 + a^2,  s = sin(th),  c = cos(th),
 //     u = k^t - a s^2 k^phi,        w = a k^t - rho k^phi
-// the contractions -Gamma^mu_ab k^a k^b collapse to (DESIGN.md "Kernel arithmetic" derives them):
+// the contractions -Gamma^mu_ab k^a k^b collapse to:
 //   dk^t  /dl = -2/Sigma^2 [ (k^r/Delta) (rho P u - 2 a s^2 r^2 Sigma k^phi) - 2 a^2 r s c k^th u ]
 //   dk^phi/dl = -2/Sigma^2 [ (k^r/Delta) (a P u + r Sigma (Sigma - 2r) k^phi)
 //                            + (c/s) k^th (Sigma^2 k^phi - 2 a r u) ]
-//   dk^r  /dl = (r - 1) (k^r)^2/Delta
-//               - 1/Sigma [ Delta (P u^2/Sigma^2 - r (s^2 (k^phi)^2 + (k^th)^2)) + r (k^r)^2
-//                           - 2 a^2 s c k^r k^th ]
+//   dk^r  /dl = (k^r)^2 [ (r - 1)/Delta - r/Sigma ]
+//               + 1/Sigma [ Delta (r (s^2 (k^phi)^2 + (k^th)^2) - P u^2/Sigma^2) + 2 a^2 s c k^r k^th ]
 //   dk^th /dl = 1/Sigma [ s c (2 r w^2/Sigma^2 + Delta (k^phi)^2 + a^2 ((k^th)^2 - (k^r)^2/Delta))
 //                         - 2 r k^r k^th ]
-// One sincos and three reciprocals (1/Sigma, 1/Delta, 1/s) per evaluation.
+// One sincos and three reciprocals (1/Sigma, 1/Delta, 1/s) per evaluation; 66 FP-pipe operations
+// (27 of them fused multiply-adds) besides the 13 of the sincos.
 //
-// Conditioning: inside the kernel the radial variable is the
-// height above the horizon  d = r - r_+  (so Delta = d (d + r_+ - r_-) keeps full relative
-// precision where the equations are singular), and the polar angle is kept in [0, pi/2] by the
-// reflection symmetry theta -> pi - theta, k^theta -> -k^theta of the Kerr metric (so the
-// absolute rounding of theta shrinks towards either pole, where the equations are singular
-// too).  Both are exact changes of variable of the same ODE; they are undone on store.
+// Conditioning: inside the kernel the radial variable is the height above
+// the horizon  d = r - r_+  (so Delta = d (d + r_+ - r_-) keeps full relative precision where the
+// equations are singular), and the polar angle is kept in [0, pi/2] by the reflection symmetry
+// theta -> pi - theta, k^theta -> -k^theta of the Kerr metric (so the absolute rounding of theta shrinks
+// towards either pole, where the equations are singular too).  Both are affine changes of variable of the
+// same ODE (they commute with RK4); they are undone on store.
 #pragma once
-#include <cuda_runtime.h>
-#include <math.h>
-#include <stdint.h>
-
-#if defined(__CUDACC__)
-#define GRAY_DEV __device__ __forceinline__
-#else
-#define GRAY_DEV inline
-#endif
+#include "gray_vec.cuh"
 
 namespace gray {
 
-template <typename T>
-struct KerrConst {
-  T a, a2;        // spin and its square
-  T rp;           // r_+ = 1 + sqrt(1 - a^2): the horizon r_bh of P:75
-  T rpm;          // r_+ - r_- = 2 sqrt(1 - a^2)
-  T h;            // step parameter (paper's Delta)
-  T r_cap, r_esc; // termination radii
+// Constants of a launch, already broadcast to V (for f2 both halves hold the same number, so the packed
+// instructions can take them straight from the constant bank / uniform registers).
+template <typename V>
+struct Consts {
+  using S = typename VT<V>::S;
+  V a, na, a2, na2, twoa2, n2a2, n2a;     // a, -a, a^2, -a^2, 2a^2, -2a^2, -2a
+  V rp, rpm, rpm1;                        // r_+ (the horizon r_bh of P:75), r_+ - r_-, r_+ - 1
+  V nh;                                   // -h (step parameter, the paper's Delta)
+  V zero, one, two, m2, half, nhalf, sixth;
+  // sin / cos (float builds): quadrant reduction and minimax polynomials, see sincos_v
+  V two_over_pi, magic, npio2_hi, npio2_lo, s1, s2, s3, c1, c2, c3, c4;
+  S r_cap, r_esc;                         // termination radii
 };
 
-// Photon state as the kernel carries it: y = (t, d, th, phi, k^t, k^r, k^th, k^phi) with d = r - r_+ and
-// th in [0, pi/2]; `mirrored` says that the true polar angle is pi - th (and the true k^theta is -k^th).
-template <typename T>
-struct Photon {
-  T y[8];
-  int mirrored;
-};
-
-// ---- scalar helpers -------------------------------------------------------------------------
-// Reciprocal.  float: MUFU.RCP (relative error <= 1 ulp, B300_MICROARCH "XU"); its three uses per
-// right-hand side sit among ~80 roundings of half an ulp each, so it is not refined.
-GRAY_DEV float rcp(float x) {
-#if defined(__CUDA_ARCH__)
-  float y;
-  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-  return y;
-#else
-  return 1.0f / x;
-#endif
+template <typename V>
+__host__ inline Consts<V> make_consts(double a, double h, double r_cap, double r_esc) {
+  using S = typename VT<V>::S;
+  Consts<V> K;
+  auto B = [](double v) { V r; S s = (S)v; S* p = (S*)&r; for (int i = 0; i < VT<V>::N; ++i) p[i] = s; return r; };
+  const double root = sqrt(1.0 - a * a);
+  K.a = B(a); K.na = B(-a); K.a2 = B(a * a); K.na2 = B(-a * a); K.twoa2 = B(2 * a * a); K.n2a2 = B(-2 * a * a);
+  K.n2a = B(-2 * a);
+  K.rp = B(1.0 + root); K.rpm = B(2.0 * root); K.rpm1 = B(root);
+  K.nh = B(-h);
+  K.zero = B(0); K.one = B(1); K.two = B(2); K.m2 = B(-2); K.half = B(0.5); K.nhalf = B(-0.5); K.sixth = B(1.0 / 6.0);
+  K.two_over_pi = B(0.636619772); K.magic = B(12582912.0);
+  K.npio2_hi = B(-1.57079637050628662109375); K.npio2_lo = B(4.371139000186241e-08);
+  K.s1 = B(-1.666666418e-01); K.s2 = B(8.332700469e-03); K.s3 = B(-1.957778732e-04);
+  K.c1 = B(-0.5); K.c2 = B(4.166664928e-02); K.c3 = B(-1.388748409e-03); K.c4 = B(2.445036807e-05);
+  K.r_cap = (S)r_cap; K.r_esc = (S)r_esc;
+  return K;
 }
-GRAY_DEV double rcp(double x) { return 1.0 / x; }
 
-// sin and cos of x for |x| < ~100 (the kernel's theta stays within a step of [0, pi/2]).
-// float: quadrant j = rint(x 2/pi) by the add-magic-constant trick, r = x - j pi/2 with pi/2 split in
-// two floats (exact enough for small |j|), then near-minimax polynomials on [-pi/4, pi/4] fitted for
-// this kernel (max error 0.86 ulp for both, checked against fp64 over 2e6 points); no slow path, no
-// int<->float conversions (those run on the quarter-rate XU pipe).
-GRAY_DEV void sincos_t(float x, float* s, float* c) {
-#if defined(__CUDA_ARCH__)
-  const float q = fmaf(x, 0.636619772f, 12582912.0f);      // 1.5 * 2^23: the low mantissa bits of q hold j
+// ---- sin and cos ---------------------------------------------------------------------------------------
+// float builds, |x| < ~100 (the kernel's theta stays within a step of [0, pi/2]): quadrant
+// j = rint(x 2/pi) by the add-magic-constant trick (1.5 * 2^23: the low mantissa bits of q hold j),
+// r = x - j pi/2 with pi/2 split in two floats, then near-minimax polynomials on [-pi/4, pi/4] fitted
+// for this kernel (max error 0.86 ulp for both, checked against fp64 over 2e6 points); no slow path and
+// no int<->float conversions.  13 FP-pipe operations; the quadrant logic is sign-bit / select work.
+GRAY_DEV void quadrant_fix(float q, float sn, float cs, float& s, float& c) {
   const int j = __float_as_int(q);
-  const float jf = q - 12582912.0f;
-  float r = fmaf(jf, -1.57079637050628662109375f, x);      // float(pi/2)
-  r = fmaf(jf, 4.371139000186241e-08f, r);                 // pi/2 - float(pi/2)
-  const float u = r * r;
-  const float sp = fmaf(fmaf(-1.957778732e-04f, u, 8.332700469e-03f), u, -1.666666418e-01f);
-  const float sn = fmaf(r * u, sp, r);
-  const float cp = fmaf(fmaf(fmaf(2.445036807e-05f, u, -1.388748409e-03f), u, 4.166664928e-02f), u, -0.5f);
-  const float cs = fmaf(u, cp, 1.0f);
   const bool swap = (j & 1) != 0;
   const float ss = swap ? cs : sn, cc = swap ? sn : cs;
-  *s = __int_as_float(__float_as_int(ss) ^ ((j & 2) << 30));          // quadrants 2, 3: sin < 0
-  *c = __int_as_float(__float_as_int(cc) ^ (((j + 1) & 2) << 30));    // quadrants 1, 2: cos < 0
-#else
-  *s = sinf(x); *c = cosf(x);
-#endif
+  s = __int_as_float(__float_as_int(ss) ^ ((j & 2) << 30));          // quadrants 2, 3: sin < 0
+  c = __int_as_float(__float_as_int(cc) ^ (((j + 1) & 2) << 30));    // quadrants 1, 2: cos < 0
 }
-GRAY_DEV void sincos_t(double x, double* s, double* c) { sincos(x, s, c); }
-GRAY_DEV float abs_t(float x) { return fabsf(x); }
-GRAY_DEV double abs_t(double x) { return fabs(x); }
-GRAY_DEV float min_t(float x, float y) { return fminf(x, y); }
-GRAY_DEV double min_t(double x, double y) { return fmin(x, y); }
+template <typename V>
+GRAY_DEV void sincos_v(const Consts<V>& K, V x, V& s, V& c) {
+  const V q = vfma(x, K.two_over_pi, K.magic);
+  const V jf = vsub(q, K.magic);
+  V r = vfma(jf, K.npio2_hi, x);
+  r = vfma(jf, K.npio2_lo, r);
+  const V u = vmul(r, r);
+  const V sp = vfma(vfma(K.s3, u, K.s2), u, K.s1);
+  const V sn = vfma(vmul(r, u), sp, r);
+  const V cp = vfma(vfma(vfma(K.c4, u, K.c3), u, K.c2), u, K.c1);
+  const V cs = vfma(u, cp, K.one);
+#pragma unroll
+  for (int l = 0; l < VT<V>::N; ++l) {
+    float sl, cl;
+    quadrant_fix(vget(q, l), vget(sn, l), vget(cs, l), sl, cl);
+    vset(s, l, sl);
+    vset(c, l, cl);
+  }
+}
+template <>
+GRAY_DEV void sincos_v<double>(const Consts<double>&, double x, double& s, double& c) { sincos(x, &s, &c); }
 
 // ---- right-hand side: accelerations dk^mu/dlambda at (d = r - r_+, th) for momentum (kt, kr, kh, kp) ----
-template <typename T>
-GRAY_DEV void geodesic_accel(const KerrConst<T>& K, T d, T th, T kt, T kr, T kh, T kp,
-                             T& at, T& ar, T& ah, T& ap) {
-  T s, c;
-  sincos_t(th, &s, &c);
-  const T r = d + K.rp;
-  const T r2 = r * r, c2 = c * c, s2 = s * s, sc = s * c;
-  const T a2c2 = K.a2 * c2;
-  const T Sg = r2 + a2c2;                       // Sigma
-  const T P = r2 - a2c2;
-  const T rho = r2 + K.a2;
-  const T Dl = d * (d + K.rpm);                 // Delta = (r - r_+)(r - r_-): no cancellation at the horizon
-  const T iS = rcp(Sg), iD = rcp(Dl), is = rcp(s);
-  const T cot = c * is;
-  const T iS2 = iS * iS;
-  const T as2 = K.a * s2;
-  const T u = kt - as2 * kp;
-  const T w = K.a * kt - rho * kp;
-  const T krD = kr * iD;                        // k^r / Delta
-  const T rSg = r * Sg;
-  const T two = T(2);
-
-  const T e1 = rho * P * u - two * as2 * r * rSg * kp;
-  at = -two * iS2 * (krD * e1 - two * K.a2 * r * sc * kh * u);
-
-  const T e2 = K.a * P * u + rSg * (Sg - two * r) * kp;
-  const T e3 = Sg * Sg * kp - two * K.a * r * u;
-  ap = -two * iS2 * (krD * e2 + cot * kh * e3);
-
-  const T kh2 = kh * kh;
-  ar = (r - T(1)) * krD * kr -
-       iS * (Dl * (P * iS2 * u * u - r * (s2 * kp * kp + kh2)) + r * kr * kr - two * K.a2 * sc * kr * kh);
-
-  ah = iS * (sc * (two * r * iS2 * w * w + Dl * kp * kp + K.a2 * (kh2 - krD * kr)) - two * r * kr * kh);
+// out[i] = dk^i/dlambda (i = t, r, th, phi) if !ACC, else add[i] + dk^i/dlambda with the addition fused into the
+// last multiply of each component (stage 4 of RK4 needs only that sum).  No addition or subtraction below
+// takes a single-use product as an operand: ptxas contracts such pairs of packed instructions into FFMA2
+// even though both carry .rn, which would make the f2 build round differently from the float build.
+template <bool ACC, typename V>
+GRAY_DEV void geodesic_accel(const Consts<V>& K, V d, V th, V kt, V kr, V kh, V kp, const V* add, V out[4]) {
+  V s, c;
+  sincos_v(K, th, s, c);
+  const V r = vadd(d, K.rp);
+  const V r2 = vmul(r, r);
+  const V c2 = vmul(c, c);
+  const V Sg = vfma(K.a2, c2, r2);              // Sigma
+  const V P = vfma(K.na2, c2, r2);
+  const V rho = vadd(r2, K.a2);
+  const V Dl = vmul(d, vadd(d, K.rpm));         // Delta = (r - r_+)(r - r_-): no cancellation at the horizon
+  const V iS = vrcp(Sg), iD = vrcp(Dl), is = vrcp(s);
+  const V niS = vneg(iS);
+  const V s2 = vmul(s, s);
+  const V sc = vmul(s, c);
+  const V as2n = vmul(K.na, s2);                // -a s^2
+  const V u = vfma(as2n, kp, kt);
+  const V krD = vmul(kr, iD);                   // k^r / Delta
+  const V niS2 = vmul(iS, niS);                 // -1/Sigma^2
+  const V tiS2 = vadd(niS2, niS2);              // -2/Sigma^2
+  const V Pu = vmul(P, u);
+  const V Sgk = vmul(Sg, kp);
+  const V rSgk = vmul(r, Sgk);
+  const V ru = vmul(r, u);
+  // dk^t
+  const V e1 = vfma(K.two, vmul(vmul(as2n, r), rSgk), vmul(rho, Pu));
+  const V tk = vmul(sc, kh);
+  const V Xt = vfma(K.n2a2, vmul(ru, tk), vmul(krD, e1));
+  out[0] = ACC ? vfma(tiS2, Xt, add[0]) : vmul(tiS2, Xt);
+  // dk^phi
+  const V e2 = vfma(K.a, Pu, vmul(vfma(K.m2, r, Sg), rSgk));
+  const V e3 = vfma(K.n2a, ru, vmul(Sg, Sgk));
+  const V ck = vmul(vmul(c, is), kh);
+  const V Xp = vfma(ck, e3, vmul(krD, e2));
+  out[3] = ACC ? vfma(tiS2, Xp, add[3]) : vmul(tiS2, Xp);
+  // dk^r
+  const V krkr = vmul(kr, kr);
+  const V G = vfma(vadd(d, K.rpm1), iD, vmul(r, niS));      // (r - 1)/Delta - r/Sigma
+  const V kp2 = vmul(kp, kp), kh2 = vmul(kh, kh);
+  const V rA1 = vmul(r, vfma(s2, kp2, kh2));
+  const V Bp = vfma(vmul(Pu, u), niS2, rA1);
+  const V J2 = vfma(K.twoa2, vmul(tk, kr), vmul(Dl, Bp));
+  out[1] = vfma(krkr, G, ACC ? vfma(iS, J2, add[1]) : vmul(iS, J2));
+  // dk^theta
+  const V w = vfma(K.na, u, Sgk);                           // rho k^phi - a k^t  (= Sigma k^phi - a u)
+  const V a2z1 = vfma(K.na2, vmul(krD, kr), vmul(K.a2, kh2));
+  const V z2 = vfma(Dl, kp2, a2z1);
+  const V z3 = vfma(vmul(r, vmul(w, w)), vneg(tiS2), z2);
+  const V z5 = vfma(K.m2, vmul(vmul(r, kr), kh), vmul(sc, z3));
+  out[2] = ACC ? vfma(iS, z5, add[2]) : vmul(iS, z5);
 }
 
 // ---- step size (gray.h gray_step_rule; paper eq. (2)) -----------------------------------------
-// y[1] = d = r - r_+.  float: the two quotients of eq. (2) are formed with MUFU.RCP (1 ulp): the step
+// Returns dlambda < 0.  float builds form the two quotients of eq. (2) with MUFU.RCP (1 ulp): the step
 // size is a free parameter of the scheme, an ulp of it is far below the truncation error it controls.
-template <typename T, int RULE>
-GRAY_DEV T step_size(const KerrConst<T>& K, const T y[8]) {
-  const T r = y[1] + K.rp;
-  if (RULE == 0) return -K.h * r;
-  const T akr = abs_t(y[5]);
-  if (sizeof(T) == 4) {
-    const T d1 = K.h * r * rcp(akr + r * (abs_t(y[6]) + abs_t(y[7])));
-    const T d2 = T(0.5) * y[1] * rcp(akr);
-    return -min_t(d1, d2);
-  }
-  const T d1 = K.h / (akr / r + abs_t(y[6]) + abs_t(y[7]));
-  const T d2 = y[1] / (T(2) * akr);
-  return -(d1 < d2 ? d1 : d2);
+template <typename V, int RULE>
+GRAY_DEV V step_size(const Consts<V>& K, V d, V kr, V kh, V kp) {
+  const V r = vadd(d, K.rp);
+  const V nhr = vmul(K.nh, r);
+  if (RULE == 0) return nhr;
+  const V akr = vabs(kr);
+  const V den = vfma(r, vadd(vabs(kh), vabs(kp)), akr);       // r (|k^r|/r + |k^th| + |k^phi|)
+  const V d1 = vmul(nhr, vrcp(den));
+  const V d2 = vmul(vmul(K.nhalf, d), vrcp(akr));
+  return vmax(d1, d2);
 }
 
 // ---- one classical RK4 step of y = (t, d, th, phi, k^t, k^r, k^th, k^phi) -------------------
-// `comp` carries, for the float build, the rounding error of each state update into the next one
+// `comp` carries, for the float builds, the rounding error of each state update into the next one
 // (compensated summation): y + comp is the state to roughly twice the working precision.
-template <typename T>
-GRAY_DEV void rk4_step(const KerrConst<T>& K, T y[8], T comp[8], T dl) {
-  T acc[8], w[8], f[4];
-  const T hdl = T(0.5) * dl;
+template <typename V>
+GRAY_DEV void rk4_step(const Consts<V>& K, V y[8], V comp[8], V dl) {
+  V acc[8], w[8], f[4];
+  const V hdl = vmul(K.half, dl);
   // stage 1
-  geodesic_accel(K, y[1], y[2], y[4], y[5], y[6], y[7], f[0], f[1], f[2], f[3]);
+  geodesic_accel<false>(K, y[1], y[2], y[4], y[5], y[6], y[7], (const V*)nullptr, f);
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
     acc[i] = y[4 + i];
     acc[4 + i] = f[i];
-    w[i] = y[i] + hdl * y[4 + i];
-    w[4 + i] = y[4 + i] + hdl * f[i];
+    w[i] = vfma(hdl, y[4 + i], y[i]);
+    w[4 + i] = vfma(hdl, f[i], y[4 + i]);
   }
-  // stage 2
-  geodesic_accel(K, w[1], w[2], w[4], w[5], w[6], w[7], f[0], f[1], f[2], f[3]);
+  // stages 2 and 3
 #pragma unroll
-  for (int i = 0; i < 4; ++i) {
-    acc[i] += T(2) * w[4 + i];
-    acc[4 + i] += T(2) * f[i];
-    const T kx = w[4 + i];
-    w[i] = y[i] + hdl * kx;
-    w[4 + i] = y[4 + i] + hdl * f[i];
-  }
-  // stage 3
-  geodesic_accel(K, w[1], w[2], w[4], w[5], w[6], w[7], f[0], f[1], f[2], f[3]);
-#pragma unroll
-  for (int i = 0; i < 4; ++i) {
-    acc[i] += T(2) * w[4 + i];
-    acc[4 + i] += T(2) * f[i];
-    const T kx = w[4 + i];
-    w[i] = y[i] + dl * kx;
-    w[4 + i] = y[4 + i] + dl * f[i];
-  }
-  // stage 4
-  geodesic_accel(K, w[1], w[2], w[4], w[5], w[6], w[7], f[0], f[1], f[2], f[3]);
-  const T dl6 = dl * T(1.0 / 6.0);
-  if (sizeof(T) == 4) {
-#pragma unroll
-    for (int i = 0; i < 8; ++i) {
-      const T inc = dl6 * (acc[i] + (i < 4 ? w[4 + i] : f[i - 4])) + comp[i];
-      const T s = y[i] + inc;
-      comp[i] = inc - (s - y[i]);          // Fast2Sum: exact whenever |y| >= |inc|
-      y[i] = s;
-    }
-  } else {
+  for (int stage = 2; stage <= 3; ++stage) {
+    const V hs = stage == 2 ? hdl : dl;
+    geodesic_accel<false>(K, w[1], w[2], w[4], w[5], w[6], w[7], (const V*)nullptr, f);
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-      y[i] += dl6 * (acc[i] + w[4 + i]);
-      y[4 + i] += dl6 * (acc[4 + i] + f[i]);
+      const V kx = w[4 + i];
+      acc[i] = vfma(K.two, kx, acc[i]);
+      acc[4 + i] = vfma(K.two, f[i], acc[4 + i]);
+      w[i] = vfma(hs, kx, y[i]);
+      w[4 + i] = vfma(hs, f[i], y[4 + i]);
+    }
+  }
+  // stage 4: the sums k1 + 2 k2 + 2 k3 + k4
+#pragma unroll
+  for (int i = 0; i < 4; ++i) acc[i] = vadd(acc[i], w[4 + i]);
+  geodesic_accel<true>(K, w[1], w[2], w[4], w[5], w[6], w[7], acc + 4, acc + 4);
+  const V dl6 = vmul(K.sixth, dl);
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    if (sizeof(typename VT<V>::S) == 4) {
+      const V inc = vfma(dl6, acc[i], comp[i]);
+      const V s = vadd(y[i], inc);
+      comp[i] = vsub(inc, vsub(s, y[i]));      // Fast2Sum: exact whenever |y| >= |inc|
+      y[i] = s;
+    } else {
+      y[i] = vfma(dl6, acc[i], y[i]);
     }
   }
 }
 
 // pi and 2 pi minus x with pi split in two parts of the working precision
-GRAY_DEV float pi_minus(float x) { return (3.14159274101257324219f - x) - 8.742278000372485e-08f; }
+GRAY_DEV float pi_minus(float x) { return __fsub_rn(__fsub_rn(3.14159274101257324219f, x), 8.742278000372485e-08f); }
 GRAY_DEV double pi_minus(double x) { return (3.141592653589793116 - x) + 1.2246467991473532e-16; }
-GRAY_DEV float two_pi_minus(float x) { return (6.28318548202514648438f - x) - 1.748455600074497e-07f; }
+GRAY_DEV float two_pi_minus(float x) { return __fsub_rn(__fsub_rn(6.28318548202514648438f, x), 1.748455600074497e-07f); }
 GRAY_DEV double two_pi_minus(double x) { return (6.283185307179586232 - x) + 2.4492935982947064e-16; }
 
 // ---- theta remap, paper eq. (3), followed by the reflection that keeps th in [0, pi/2] ----------
-// Eq. (3) acts on the true polar angle.  For a mirrored photon (true angle pi - th) the true angle
-// exceeds pi when th < 0 and is negative when th > pi, so the sign of the phi shift flips with it.
-template <typename T>
-GRAY_DEV void remap_theta(T y[8], T comp[8], int& mirrored) {
-  const T pi = T(3.14159265358979323846);
-  const T shift = mirrored ? -pi : pi;
-  if (y[2] > pi) {
-    y[2] = two_pi_minus(y[2]);
-    y[3] += shift;
-    y[6] = -y[6];
-    comp[2] = -comp[2]; comp[6] = -comp[6];
-  } else if (y[2] < T(0)) {
-    y[2] = -y[2];
-    y[3] -= shift;
-    y[6] = -y[6];
-    comp[2] = -comp[2]; comp[6] = -comp[6];
+// One photon (scalar S).  Eq. (3) acts on the true polar angle.  For a mirrored photon (true angle
+// pi - th) the true angle exceeds pi when th < 0 and is negative when th > pi, so the sign of the phi
+// shift flips with it.
+template <typename S>
+GRAY_DEV void remap_theta(S& th, S& ph, S& kh, S& c_th, S& c_kh, int& mirrored) {
+  const S pi = S(3.14159265358979323846);
+  const S shift = mirrored ? -pi : pi;
+  if (th > pi) {
+    th = two_pi_minus(th);
+    ph += shift;
+    kh = sneg(kh); c_th = sneg(c_th); c_kh = sneg(c_kh);
+  } else if (th < S(0)) {
+    th = sneg(th);
+    ph -= shift;
+    kh = sneg(kh); c_th = sneg(c_th); c_kh = sneg(c_kh);
   }
-  if (y[2] > T(1.57079632679489661923)) {
-    y[2] = pi_minus(y[2]);
-    y[6] = -y[6];
-    comp[2] = -comp[2]; comp[6] = -comp[6];
+  if (th > S(1.57079632679489661923)) {
+    th = pi_minus(th);
+    kh = sneg(kh); c_th = sneg(c_th); c_kh = sneg(c_kh);
     mirrored ^= 1;
   }
 }
 
-// ---- status of a state after a full step: BAD(3) / CAPTURED(1) / ESCAPED(2) / LIVE(0), in that order
-template <typename T>
-GRAY_DEV int state_status(const KerrConst<T>& K, const T y[8]) {
-  T z = T(0);
+// ---- non-finite detector: z = sum_i 0 * y_i is 0 iff all eight components are finite -----------------
+template <typename V>
+GRAY_DEV V nonfinite_probe(const Consts<V>& K, const V y[8]) {
+  V z = vmul(K.zero, y[0]);
 #pragma unroll
-  for (int i = 0; i < 8; ++i) z += T(0) * y[i];     // inf * 0 = NaN, NaN * 0 = NaN, finite * 0 = 0
-  if (!(z == T(0))) return 3;
-  const T r = y[1] + K.rp;
-  if (r < K.r_cap) return 1;
-  if (r > K.r_esc) return 2;
+  for (int i = 1; i < 8; ++i) z = vfma(K.zero, y[i], z);
+  return z;
+}
+
+// status of one photon after a full step: BAD(3) / CAPTURED(1) / ESCAPED(2) / LIVE(0), in that order
+template <typename S>
+GRAY_DEV int state_status(S z, S r, S r_cap, S r_esc) {
+  if (!(z == S(0))) return 3;
+  if (r < r_cap) return 1;
+  if (r > r_esc) return 2;
   return 0;
 }
 

@@ -32,7 +32,8 @@ class _State(C.Structure):
 class _StepParams(C.Structure):
     _fields_ = [("h", C.c_double), ("r_capture_factor", C.c_double), ("horizon_delta", C.c_double),
                 ("r_escape_factor", C.c_double), ("rule", C.c_int32), ("schedule", C.c_int32),
-                ("refill_interval", C.c_int32), ("frozen", C.c_int32)]
+                ("refill_interval", C.c_int32), ("frozen", C.c_int32), ("photons_per_thread", C.c_int32),
+                ("reserved", C.c_int32)]
 
 
 class _Counters(C.Structure):
@@ -99,9 +100,9 @@ class StepParams:
     """gray_step_params (include/gray.h).  Defaults: the BASELINE configs' h, capture and escape radii."""
 
     def __init__(self, h=1.0 / 32, r_capture_factor=1.01, horizon_delta=1e-6, r_escape_factor=1.01, rule=STEP_EQ2,
-                 schedule=SCHED_REFILL, refill_interval=0, frozen=False):
+                 schedule=SCHED_REFILL, refill_interval=0, frozen=False, photons_per_thread=0):
         self.c = _StepParams(h, r_capture_factor, horizon_delta, r_escape_factor, rule, schedule, refill_interval,
-                             int(bool(frozen)))
+                             int(bool(frozen)), photons_per_thread, 0)
 
 
 class PhotonBatch:

@@ -152,7 +152,9 @@ def test_schedules_intervals_and_resume_are_bit_identical():
     for prec in (g.GRAY_F32, g.GRAY_F64):
         base = None
         for kw in (dict(schedule=g.SCHED_REFILL, refill_interval=8), dict(schedule=g.SCHED_REFILL, refill_interval=1),
-                   dict(schedule=g.SCHED_REFILL, refill_interval=37), dict(schedule=g.SCHED_STATIC)):
+                   dict(schedule=g.SCHED_REFILL, refill_interval=37), dict(schedule=g.SCHED_STATIC),
+                   # one photon per thread (scalar FFMA) vs the default two (packed FFMA2): same bits per photon
+                   dict(schedule=g.SCHED_REFILL, photons_per_thread=1), dict(schedule=g.SCHED_STATIC, photons_per_thread=1)):
             b = g.PhotonBatch(nx * ny, prec)
             g.gray_init_rays(b, a, wl.R_OBS, inc, W, nx, ny)
             g.gray_integrate(b, max_steps=wl.MAX_STEPS, params=g.StepParams(rule=g.STEP_EQ2, **kw))
