@@ -65,26 +65,38 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
 #pragma unroll
   for (int l = 0; l < N; ++l) { have[l] = false; mirrored[l] = 0; idx[l] = 0; nst[l] = nst0[l] = iss[l] = 0; fstat[l] = GRAY_LIVE; }
 
-  // HBM -> registers: photon p into slot l, if it is live and has steps left.  (t, r, theta, phi), k^mu ->
-  // the kernel's variables (gray_math.cuh): d = r - r_+ and theta folded into [0, pi/2].
-  auto take = [&](int l, unsigned long long p) {
-    const uint8_t st = A.status[p];
-    const uint32_t s = A.steps[p];
-    if (st != GRAY_LIVE) return;
-    if (s >= A.max_steps) { ++c_live; return; }
-    const typename Vec4T<S>::type xv = A.x[p], kv = A.k[p];
-    S th = xv.z, kh = kv.z;
-    int m = 0;
-    if (th > S(1.57079632679489661923)) { th = pi_minus(th); kh = sneg(kh); m = 1; }
-    vset(y[0], l, xv.x); vset(y[1], l, xv.y - vget(K.rp, 0)); vset(y[2], l, th); vset(y[3], l, xv.w);
-    vset(y[4], l, kv.x); vset(y[5], l, kv.y); vset(y[6], l, kh); vset(y[7], l, kv.w);
+  // HBM -> registers: photon want[l] into slot l (for the slots with want[l] < n), if it is live and has steps
+  // left.  (t, r, theta, phi), k^mu -> the kernel's variables (gray_math.cuh): d = r - r_+ and theta folded into
+  // [0, pi/2].  The state is taken apart into scalars, the slots are filled under their own conditions, and it is
+  // put together again unconditionally: a packed value is never half-updated inside a branch.
+  auto take = [&](const unsigned long long want[N]) {
+    S ys[8][N], cs[8][N];
 #pragma unroll
-    for (int i = 0; i < 8; ++i) vset(comp[i], l, S(0));
-    mirrored[l] = m;
-    idx[l] = p;
-    nst[l] = nst0[l] = iss[l] = s;
-    fstat[l] = GRAY_LIVE;
-    have[l] = true;
+    for (int i = 0; i < 8; ++i) { vunpack(y[i], ys[i]); vunpack(comp[i], cs[i]); }
+#pragma unroll
+    for (int l = 0; l < N; ++l) {
+      const unsigned long long p = want[l];
+      if (p >= A.n) continue;
+      const uint8_t st = A.status[p];
+      const uint32_t s = A.steps[p];
+      if (st != GRAY_LIVE) continue;
+      if (s >= A.max_steps) { ++c_live; continue; }
+      const typename Vec4T<S>::type xv = A.x[p], kv = A.k[p];
+      S th = xv.z, kh = kv.z;
+      int m = 0;
+      if (th > S(1.57079632679489661923)) { th = pi_minus(th); kh = sneg(kh); m = 1; }
+      ys[0][l] = xv.x; ys[1][l] = xv.y - vget(K.rp, 0); ys[2][l] = th; ys[3][l] = xv.w;
+      ys[4][l] = kv.x; ys[5][l] = kv.y; ys[6][l] = kh; ys[7][l] = kv.w;
+#pragma unroll
+      for (int i = 0; i < 8; ++i) cs[i][l] = S(0);
+      mirrored[l] = m;
+      idx[l] = p;
+      nst[l] = nst0[l] = iss[l] = s;
+      fstat[l] = GRAY_LIVE;
+      have[l] = true;
+    }
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { vpack(y[i], ys[i]); vpack(comp[i], cs[i]); }
   };
   // registers -> HBM
   auto retire = [&](int l, int st) {
@@ -103,11 +115,10 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
   };
 
   if (SCHED == GRAY_SCHED_STATIC) {
+    unsigned long long want[N];
 #pragma unroll
-    for (int l = 0; l < N; ++l) {
-      const unsigned long long p = ((unsigned long long)blockIdx.x * N + l) * kBlock + threadIdx.x;
-      if (p < A.n) take(l, p);
-    }
+    for (int l = 0; l < N; ++l) want[l] = ((unsigned long long)blockIdx.x * N + l) * kBlock + threadIdx.x;
+    take(want);
   }
 
   for (;;) {
@@ -120,15 +131,14 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
         unsigned long long base = 0;
         if (lane == 0) base = atomicAdd(&A.ws->queue_head, (unsigned long long)cnt);
         base = __shfl_sync(FULL, base, 0);
+        unsigned long long want[N];
         int off = 0;
 #pragma unroll
         for (int l = 0; l < N; ++l) {
-          if (!have[l]) {
-            const unsigned long long p = base + off + __popc(need[l] & ((1u << lane) - 1u));
-            if (p < A.n) take(l, p);
-          }
+          want[l] = have[l] ? ~0ull : base + off + __popc(need[l] & ((1u << lane) - 1u));
           off += __popc(need[l]);
         }
+        take(want);
         if (base + cnt >= A.n) exhausted = true;
       }
     }
@@ -149,12 +159,16 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
           rk4_step(K, y, comp, dl);
           const V z = nonfinite_probe(K, y);
           const V r = vadd(y[1], K.rp);
+          // eq. (3) remap and the fold, on the scalars of every slot (a slot without a photon carries junk,
+          // which is remapped too and never stored), then the packed values are rebuilt unconditionally
+          S th[N], ph[N], kh[N], c2[N], c6[N];
+          vunpack(y[2], th); vunpack(y[3], ph); vunpack(y[6], kh); vunpack(comp[2], c2); vunpack(comp[6], c6);
+#pragma unroll
+          for (int l = 0; l < N; ++l) remap_theta(th[l], ph[l], kh[l], c2[l], c6[l], mirrored[l]);
+          vpack(y[2], th); vpack(y[3], ph); vpack(y[6], kh); vpack(comp[2], c2); vpack(comp[6], c6);
 #pragma unroll
           for (int l = 0; l < N; ++l) {
             if (have[l]) {
-              S th = vget(y[2], l), ph = vget(y[3], l), kh = vget(y[6], l), c2 = vget(comp[2], l), c6 = vget(comp[6], l);
-              remap_theta(th, ph, kh, c2, c6, mirrored[l]);
-              vset(y[2], l, th); vset(y[3], l, ph); vset(y[6], l, kh); vset(comp[2], l, c2); vset(comp[6], l, c6);
               ++nst[l];
               const int st = state_status(vget(z, l), vget(r, l), K.r_cap, K.r_esc);
               if (st != GRAY_LIVE || nst[l] == A.max_steps) retire(l, st);
@@ -167,23 +181,33 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
           rk4_step(K, w, wc, dl);
           const V z = nonfinite_probe(K, w);
           const V r = vadd(w[1], K.rp);
+          S th[N], ph[N], kh[N], c2[N], c6[N];
+          int wm[N];
+          bool adv[N];
+          vunpack(w[2], th); vunpack(w[3], ph); vunpack(w[6], kh); vunpack(wc[2], c2); vunpack(wc[6], c6);
+#pragma unroll
+          for (int l = 0; l < N; ++l) {
+            wm[l] = mirrored[l];
+            remap_theta(th[l], ph[l], kh[l], c2[l], c6[l], wm[l]);
+            adv[l] = have[l] && fstat[l] == GRAY_LIVE;
+          }
+          vpack(w[2], th); vpack(w[3], ph); vpack(w[6], kh); vpack(wc[2], c2); vpack(wc[6], c6);
+          // frozen by select: a slot advances only while its photon is live
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            S a[N], b[N], ca[N], cb[N];
+            vunpack(y[i], a); vunpack(w[i], b); vunpack(comp[i], ca); vunpack(wc[i], cb);
+#pragma unroll
+            for (int l = 0; l < N; ++l) { a[l] = adv[l] ? b[l] : a[l]; ca[l] = adv[l] ? cb[l] : ca[l]; }
+            vpack(y[i], a); vpack(comp[i], ca);
+          }
 #pragma unroll
           for (int l = 0; l < N; ++l) {
             if (have[l]) {
-              S th = vget(w[2], l), ph = vget(w[3], l), kh = vget(w[6], l), c2 = vget(wc[2], l), c6 = vget(wc[6], l);
-              int wm = mirrored[l];
-              remap_theta(th, ph, kh, c2, c6, wm);
-              vset(w[2], l, th); vset(w[3], l, ph); vset(w[6], l, kh); vset(wc[2], l, c2); vset(wc[6], l, c6);
               const int st = state_status(vget(z, l), vget(r, l), K.r_cap, K.r_esc);
-              const bool adv = (fstat[l] == GRAY_LIVE);
-#pragma unroll
-              for (int i = 0; i < 8; ++i) {
-                vset(y[i], l, adv ? vget(w[i], l) : vget(y[i], l));
-                vset(comp[i], l, adv ? vget(wc[i], l) : vget(comp[i], l));
-              }
-              mirrored[l] = adv ? wm : mirrored[l];
-              nst[l] += adv ? 1u : 0u;
-              fstat[l] = adv ? st : fstat[l];
+              mirrored[l] = adv[l] ? wm[l] : mirrored[l];
+              nst[l] += adv[l] ? 1u : 0u;
+              fstat[l] = adv[l] ? st : fstat[l];
               ++iss[l];
               if (iss[l] == A.max_steps) retire(l, fstat[l]);
             }

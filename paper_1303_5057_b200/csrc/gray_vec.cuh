@@ -18,7 +18,16 @@
 
 namespace gray {
 
-struct f2 { float x, y; };
+// Two floats in one 64-bit register pair (x = photon 0 in the low word, y = photon 1 in the high word).  Held as
+// a single 64-bit value so that the register allocator keeps the pair together across the loop: the packed
+// instructions need an aligned pair, and assembling one from two free-floating scalars costs a MOV per half.
+struct f2 { unsigned long long v; };
+GRAY_DEV f2 f2_pack(float lo, float hi) {
+  f2 r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r.v) : "f"(lo), "f"(hi));
+  return r;
+}
+GRAY_DEV void f2_unpack(f2 a, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a.v)); }
 
 template <typename V> struct VT;
 template <> struct VT<float>  { using S = float;  static constexpr int N = 1; };
@@ -29,14 +38,21 @@ template <> struct VT<f2>     { using S = float;  static constexpr int N = 2; };
 template <typename V> GRAY_DEV V vsplat(typename VT<V>::S s);
 template <> GRAY_DEV float vsplat<float>(float s) { return s; }
 template <> GRAY_DEV double vsplat<double>(double s) { return s; }
-template <> GRAY_DEV f2 vsplat<f2>(float s) { f2 r; r.x = s; r.y = s; return r; }
+template <> GRAY_DEV f2 vsplat<f2>(float s) { return f2_pack(s, s); }
 
 GRAY_DEV float vget(float v, int) { return v; }
 GRAY_DEV double vget(double v, int) { return v; }
-GRAY_DEV float vget(f2 v, int l) { return l ? v.y : v.x; }
+GRAY_DEV float vget(f2 v, int l) { float lo, hi; f2_unpack(v, lo, hi); return l ? hi : lo; }
 GRAY_DEV void vset(float& v, int, float s) { v = s; }
 GRAY_DEV void vset(double& v, int, double s) { v = s; }
-GRAY_DEV void vset(f2& v, int l, float s) { if (l) v.y = s; else v.x = s; }
+GRAY_DEV void vset(f2& v, int l, float s) { float lo, hi; f2_unpack(v, lo, hi); v = l ? f2_pack(lo, s) : f2_pack(s, hi); }
+// all lanes at once: v <-> s[0 .. N-1]
+GRAY_DEV void vunpack(float v, float s[1]) { s[0] = v; }
+GRAY_DEV void vunpack(double v, double s[1]) { s[0] = v; }
+GRAY_DEV void vunpack(f2 v, float s[2]) { f2_unpack(v, s[0], s[1]); }
+GRAY_DEV void vpack(float& v, const float s[1]) { v = s[0]; }
+GRAY_DEV void vpack(double& v, const double s[1]) { v = s[0]; }
+GRAY_DEV void vpack(f2& v, const float s[2]) { v = f2_pack(s[0], s[1]); }
 
 // ---- add, sub, mul, fma: one rounding each -----------------------------------------------------------
 GRAY_DEV float vadd(float a, float b) { return __fadd_rn(a, b); }
@@ -56,13 +72,11 @@ GRAY_DEV double vsub(double a, double b) {
 GRAY_DEV double vmul(double a, double b) { return __dmul_rn(a, b); }
 GRAY_DEV double vfma(double a, double b, double c) { return __fma_rn(a, b, c); }
 
-#define GRAY_F2_BINARY(name, op)                                                                     \
-  GRAY_DEV f2 name(f2 a, f2 b) {                                                                     \
-    f2 d;                                                                                            \
-    asm("{\n\t.reg .b64 ra, rb, rd;\n\tmov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %5};\n\t" op        \
-        " rd, ra, rb;\n\tmov.b64 {%0, %1}, rd;\n\t}"                                                 \
-        : "=f"(d.x), "=f"(d.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));                            \
-    return d;                                                                                        \
+#define GRAY_F2_BINARY(name, op)                                                     \
+  GRAY_DEV f2 name(f2 a, f2 b) {                                                     \
+    f2 d;                                                                            \
+    asm(op " %0, %1, %2;" : "=l"(d.v) : "l"(a.v), "l"(b.v));                         \
+    return d;                                                                        \
   }
 GRAY_F2_BINARY(vadd, "add.rn.f32x2")
 GRAY_F2_BINARY(vsub, "sub.rn.f32x2")
@@ -70,9 +84,7 @@ GRAY_F2_BINARY(vmul, "mul.rn.f32x2")
 #undef GRAY_F2_BINARY
 GRAY_DEV f2 vfma(f2 a, f2 b, f2 c) {
   f2 d;
-  asm("{\n\t.reg .b64 ra, rb, rc, rd;\n\tmov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %5};\n\tmov.b64 rc, {%6, %7};\n\t"
-      "fma.rn.f32x2 rd, ra, rb, rc;\n\tmov.b64 {%0, %1}, rd;\n\t}"
-      : "=f"(d.x), "=f"(d.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y), "f"(c.x), "f"(c.y));
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d.v) : "l"(a.v), "l"(b.v), "l"(c.v));
   return d;
 }
 
@@ -83,10 +95,10 @@ GRAY_DEV double sneg(double x) { return -x; }
 GRAY_DEV double sabs(double x) { return fabs(x); }
 GRAY_DEV float vneg(float x) { return sneg(x); }
 GRAY_DEV double vneg(double x) { return -x; }
-GRAY_DEV f2 vneg(f2 v) { f2 r; r.x = sneg(v.x); r.y = sneg(v.y); return r; }
+GRAY_DEV f2 vneg(f2 v) { float lo, hi; f2_unpack(v, lo, hi); return f2_pack(sneg(lo), sneg(hi)); }
 GRAY_DEV float vabs(float x) { return sabs(x); }
 GRAY_DEV double vabs(double x) { return fabs(x); }
-GRAY_DEV f2 vabs(f2 v) { f2 r; r.x = sabs(v.x); r.y = sabs(v.y); return r; }
+GRAY_DEV f2 vabs(f2 v) { float lo, hi; f2_unpack(v, lo, hi); return f2_pack(sabs(lo), sabs(hi)); }
 
 // ---- reciprocal -------------------------------------------------------------------------------------
 // float: MUFU.RCP (relative error <= 1 ulp); its uses sit among ~80 half-ulp roundings per right-hand
@@ -98,11 +110,16 @@ GRAY_DEV float srcp(float x) {
 }
 GRAY_DEV float vrcp(float x) { return srcp(x); }
 GRAY_DEV double vrcp(double x) { return __drcp_rn(x); }
-GRAY_DEV f2 vrcp(f2 v) { f2 r; r.x = srcp(v.x); r.y = srcp(v.y); return r; }
+GRAY_DEV f2 vrcp(f2 v) { float lo, hi; f2_unpack(v, lo, hi); return f2_pack(srcp(lo), srcp(hi)); }
 
 // ---- min / max (ALU pipe for float) --------------------------------------------------------------------
 GRAY_DEV float vmax(float a, float b) { return fmaxf(a, b); }
 GRAY_DEV double vmax(double a, double b) { return fmax(a, b); }
-GRAY_DEV f2 vmax(f2 a, f2 b) { f2 r; r.x = fmaxf(a.x, b.x); r.y = fmaxf(a.y, b.y); return r; }
+GRAY_DEV f2 vmax(f2 a, f2 b) {
+  float al, ah, bl, bh;
+  f2_unpack(a, al, ah);
+  f2_unpack(b, bl, bh);
+  return f2_pack(fmaxf(al, bl), fmaxf(ah, bh));
+}
 
 }  // namespace gray
