@@ -30,10 +30,16 @@ struct IntegrateArgs {
   Consts<V> K;
 };
 
-constexpr int kBlock = 128;
+#ifndef GRAY_BLOCK
+#define GRAY_BLOCK 128
+#endif
+#ifndef GRAY_F2_MIN_BLOCKS
+#define GRAY_F2_MIN_BLOCKS 4
+#endif
+constexpr int kBlock = GRAY_BLOCK;
 template <typename V> struct Tune;
 template <> struct Tune<float> { static constexpr int min_blocks = 4; };    // <= 128 registers/thread
-template <> struct Tune<f2> { static constexpr int min_blocks = 4; };       // <= 128 registers/thread
+template <> struct Tune<f2> { static constexpr int min_blocks = GRAY_F2_MIN_BLOCKS; };   // 4 x 128 threads: <= 128 registers/thread
 template <> struct Tune<double> { static constexpr int min_blocks = 2; };   // <= 255 registers/thread
 
 __device__ __forceinline__ unsigned long long warp_sum(unsigned long long v) {
@@ -159,20 +165,33 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
           rk4_step(K, y, comp, dl);
           const V z = nonfinite_probe(K, y);
           const V r = vadd(y[1], K.rp);
-          // eq. (3) remap and the fold, on the scalars of every slot (a slot without a photon carries junk,
-          // which is remapped too and never stored), then the packed values are rebuilt unconditionally
-          S th[N], ph[N], kh[N], c2[N], c6[N];
-          vunpack(y[2], th); vunpack(y[3], ph); vunpack(y[6], kh); vunpack(comp[2], c2); vunpack(comp[6], c6);
+          // Bookkeeping.  Common case first, with one branch for the whole thread: every slot's theta still in
+          // [0, pi/2] (no eq. (3) remap, no fold) and no slot finished.
+          S th[N], rr[N], zz[N];
+          vunpack(y[2], th); vunpack(r, rr); vunpack(z, zz);
+          bool out_of_fold = false;
 #pragma unroll
-          for (int l = 0; l < N; ++l) remap_theta(th[l], ph[l], kh[l], c2[l], c6[l], mirrored[l]);
-          vpack(y[2], th); vpack(y[3], ph); vpack(y[6], kh); vpack(comp[2], c2); vpack(comp[6], c6);
+          for (int l = 0; l < N; ++l) out_of_fold |= !(th[l] >= S(0) && th[l] <= S(1.57079632679489661923));
+          if (out_of_fold) {
+            // eq. (3) remap and the fold, on the scalars of every slot (a slot without a photon carries junk,
+            // which is remapped too and never stored), then the packed values are rebuilt unconditionally
+            S ph[N], kh[N], c2[N], c6[N];
+            vunpack(y[3], ph); vunpack(y[6], kh); vunpack(comp[2], c2); vunpack(comp[6], c6);
+#pragma unroll
+            for (int l = 0; l < N; ++l) remap_theta(th[l], ph[l], kh[l], c2[l], c6[l], mirrored[l]);
+            vpack(y[2], th); vpack(y[3], ph); vpack(y[6], kh); vpack(comp[2], c2); vpack(comp[6], c6);
+          }
+          bool fin[N], any_fin = false;
 #pragma unroll
           for (int l = 0; l < N; ++l) {
-            if (have[l]) {
-              ++nst[l];
-              const int st = state_status(vget(z, l), vget(r, l), K.r_cap, K.r_esc);
-              if (st != GRAY_LIVE || nst[l] == A.max_steps) retire(l, st);
-            }
+            ++nst[l];
+            fin[l] = have[l] && (!(zz[l] == S(0) && rr[l] >= K.r_cap && rr[l] <= K.r_esc) || nst[l] == A.max_steps);
+            any_fin |= fin[l];
+          }
+          if (any_fin) {
+#pragma unroll
+            for (int l = 0; l < N; ++l)
+              if (fin[l]) retire(l, state_status(zz[l], rr[l], K.r_cap, K.r_esc));
           }
         } else {
           V w[8], wc[8];

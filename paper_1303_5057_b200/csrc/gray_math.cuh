@@ -28,6 +28,13 @@
 #pragma once
 #include "gray_vec.cuh"
 
+// Components of y = (t, d, th, phi, k^t, k^r, k^th, k^phi) whose update is a compensated sum in the float builds
+// (bit i = component i).  t (bit 0) is left out: it feeds nothing back, and measured on B200 the final (r, theta, phi)
+// and the drift of E, L_z, Q are bit-for-bit the same with and without it.
+#ifndef GRAY_COMP_MASK
+#define GRAY_COMP_MASK 0xfe
+#endif
+
 namespace gray {
 
 // Constants of a launch, already broadcast to V (for f2 both halves hold the same number, so the packed
@@ -207,7 +214,7 @@ GRAY_DEV void rk4_step(const Consts<V>& K, V y[8], V comp[8], V dl) {
   const V dl6 = vmul(K.sixth, dl);
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
-    if (sizeof(typename VT<V>::S) == 4) {
+    if (sizeof(typename VT<V>::S) == 4 && ((GRAY_COMP_MASK >> i) & 1)) {
       const V inc = vfma(dl6, acc[i], comp[i]);
       const V s = vadd(y[i], inc);
       comp[i] = vsub(inc, vsub(s, y[i]));      // Fast2Sum: exact whenever |y| >= |inc|
@@ -248,12 +255,16 @@ GRAY_DEV void remap_theta(S& th, S& ph, S& kh, S& c_th, S& c_kh, int& mirrored) 
   }
 }
 
-// ---- non-finite detector: z = sum_i 0 * y_i is 0 iff all eight components are finite -----------------
+// ---- non-finite detector: z = sum_i 0 * k^i is 0 iff the four momentum components are finite ------------
+// The positions need no probe: x_new = x + dlambda/6 (sum of the stage momenta), and a stage momentum is
+// non-finite only if an acceleration is, which makes the new momentum non-finite as well; so with finite
+// momenta the positions stay finite (short of the overflow of a finite sum beyond 3e38, which r_escape
+// excludes).  The oracle's test on all eight components (R10) fires on the same step.
 template <typename V>
 GRAY_DEV V nonfinite_probe(const Consts<V>& K, const V y[8]) {
-  V z = vmul(K.zero, y[0]);
+  V z = vmul(K.zero, y[4]);
 #pragma unroll
-  for (int i = 1; i < 8; ++i) z = vfma(K.zero, y[i], z);
+  for (int i = 5; i < 8; ++i) z = vfma(K.zero, y[i], z);
   return z;
 }
 
