@@ -31,8 +31,10 @@ FLOPS_PER_PHOTON_STEP = {"rel": 777, "eq2": 787}
 # FP32 CUDA-core peak the integrator is bound by: 148 SMs x 128 lanes x 2 (FMA) x
 # 1.965 GHz (clocks.max.sm); FP64: 64 lanes per SM.
 PEAK_TFLOPS = {"f32": 148 * 128 * 2 * 1.965e9 / 1e12, "f64": 148 * 64 * 2 * 1.965e9 / 1e12}
-# dram bytes per gray_integrate launch from the committed `ncu --set full` capture (profiles/), per photon
-NCU_DRAM_BYTES_PER_PHOTON = None
+# dram__bytes_read.sum + dram__bytes_write.sum of one gray_integrate launch in the committed `ncu --set full`
+# capture (profiles/r01_README.md: 260.2 MB for 2^22 photons, fp32), per photon; the launch of this run is
+# scaled from it (a capture at 2^28 photons would replay a 3.7 s kernel ~40 times)
+NCU_DRAM_BYTES_PER_PHOTON = 62.04
 
 
 def parse():
@@ -51,7 +53,7 @@ def parse():
     ap.add_argument("--e2e-log2n", type=int, default=-1, help="photons per GPU of the host-buffer run (default min(log2n, 26))")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--ref-log2n", type=int, default=15, help="--impl reference: photons of the strided sample per step")
+    ap.add_argument("--ref-log2n", type=int, default=18, help="--impl reference: photons of the strided sample per step")
     return ap.parse_args()
 
 
@@ -280,7 +282,8 @@ def run_gray(args):
     peak = PEAK_TFLOPS[args.prec]
     fma_peak = g.gray_fma_peak(prec, 8192) / 1e12
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                "traffic": (NCU_DRAM_BYTES_PER_PHOTON * n) if NCU_DRAM_BYTES_PER_PHOTON else None,
+                "traffic": (NCU_DRAM_BYTES_PER_PHOTON * n) if (NCU_DRAM_BYTES_PER_PHOTON and args.prec == "f32") else None,
+                "traffic_source": "ncu dram bytes per photon at 2^22 photons x photons of this launch",
                 "kernel": "gray::integrate_kernel", "kernel_ms": kern_ms, "kernel_share_of_step": kern_ms * args.steps / ms,
                 "flops_per_photon_step": flops, "flops_source": "oracle operation tally (add=sub=mul=div=sqrt=sin=cos=1)",
                 "peak_source": "148 SMs x %d lanes x 2 x 1.965 GHz (DESIGN.md)" % (128 if args.prec == "f32" else 64),
@@ -303,7 +306,7 @@ def run_gray(args):
     if not args.no_cpu_baseline:
         import oracle as o                          # cpu_baseline leg only
         threads = max(1, o.hardware_threads())
-        ps, dt, m = oracle_sample(args, 17, threads)
+        ps, dt, m = oracle_sample(args, 18, threads)
         out["cpu_baseline"] = {"value": ps / dt, "unit": "photon-steps/s", "cores": threads, "kind": "oracle",
                                "sample": f"{m} photons, strided p = j * 2^{args.log2n} / {m} of rank 0's photons, "
                                          f"{ps} photon-steps in {dt:.1f} s", "ns_per_photon_step_per_core": 1e9 * dt * threads / ps}

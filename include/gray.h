@@ -125,6 +125,12 @@ typedef struct {
                                 FMUL2 / FADD2, GRAY_F32 only); 1 = one photon per thread, scalar
                                 instructions.  Per-photon results are bit-identical for 1 and 2.       */
   int32_t reserved;          /* must be 0                                                             */
+  double xi_epsilon;         /* > 0: the paper's production pole treatment: after every RK4 step
+                                xi of eq. (4) is evaluated at the new state; if |xi + 1| > xi_epsilon (the
+                                paper's epsilon ~ 1e-3) or xi is not finite, the step is discarded and
+                                re-integrated from the old state as ONE forward Euler step of dlambda / 9,
+                                which is not tested itself (reading R18).  0 = off.  Not available
+                                together with `frozen`.                                               */
 } gray_step_params;
 
 /* Bytes of device workspace gray_integrate / gray_classify / gray_shadow_edge need (queue head and
@@ -148,6 +154,7 @@ typedef struct {
   uint64_t issued_steps;     /* lane-steps issued by warps, including idle and frozen lanes            */
   uint64_t photons_done;     /* photons this call brought to CAPTURED / ESCAPED / BAD                  */
   uint64_t photons_live;     /* photons this call left LIVE at max_steps                               */
+  uint64_t fallback_steps;   /* steps re-integrated by the xi monitor (xi_epsilon > 0)                 */
 } gray_counters;
 
 /* Counters of the last gray_integrate on this workspace.  Synchronises the stream.                  */

@@ -275,6 +275,7 @@ struct StepParams {
   double r_capture;    // captured when r <  r_capture  (1.01 r_h in the configs; r_h + delta in P:79)
   double r_escape;     // escaped  when r >  r_escape   (1.01 r_obs)
   int rule;            // StepRule
+  double xi_eps = 0.0; // > 0: the paper's production pole treatment with epsilon = xi_eps, see integrate()
 };
 
 // Status of a state after a full step: non-finite -> BAD,
@@ -287,6 +288,27 @@ inline int classify_state(const double y[8], const StepParams& sp) {
   return LIVE;
 }
 
+// The paper's production pole treatment (NEXT-1 of SURVEY §8(f)): "monitor the quantity xi [eq. 4]
+// which should always remain equal to -1.  If |xi + 1| > epsilon, for some small parameter epsilon ~ 1e-3 ...
+// we re-integrate the inaccurate step by falling back to the 1st-order forward Euler scheme with a smaller
+// time step dlambda'/9".  xi + 1 is invariants()[3] (the null norm over g_tt (k^t)^2).  Reading (R18):
+// the test is applied to the state an RK4 step produced; on failure that step is discarded and replaced by ONE
+// forward Euler step of dlambda/9 from the state before it, which is not tested itself; a non-finite xi fails
+// the test.  One step (RK4 or its Euler replacement) counts as one step.
+inline void advance(double a, double y[8], const StepParams& sp) {
+  double dl = step_size(a, y, sp.h, sp.rule);
+  if (!(sp.xi_eps > 0.0)) { rk4_step(a, y, dl); return; }
+  double y_old[8], inv[4];
+  for (int i = 0; i < 8; ++i) y_old[i] = y[i];
+  rk4_step(a, y, dl);
+  invariants(a, y, inv);
+  if (!(fabs(inv[3]) <= sp.xi_eps)) {
+    double f[8];
+    rhs(a, y_old, f);
+    for (int i = 0; i < 8; ++i) y[i] = y_old[i] + (dl / 9.0) * f[i];
+  }
+}
+
 // Integrate one ray until it is captured, escapes, goes non-finite or has taken
 // max_steps steps in total.  *steps is the running step counter (in/out), so a
 // call can resume an earlier one.  If force_steps >= 0 the tests are ignored and
@@ -296,8 +318,7 @@ inline int integrate(double a, double y[8], const StepParams& sp, uint32_t max_s
                      int64_t force_steps, uint32_t* steps) {
   if (force_steps >= 0) {
     for (int64_t n = 0; n < force_steps; ++n) {
-      double dl = step_size(a, y, sp.h, sp.rule);
-      rk4_step(a, y, dl);
+      advance(a, y, sp);
       remap_theta(y);
       ++*steps;
     }
@@ -305,8 +326,7 @@ inline int integrate(double a, double y[8], const StepParams& sp, uint32_t max_s
   }
   int st = LIVE;
   while (*steps < max_steps) {
-    double dl = step_size(a, y, sp.h, sp.rule);
-    rk4_step(a, y, dl);
+    advance(a, y, sp);
     remap_theta(y);
     ++*steps;
     st = classify_state(y, sp);

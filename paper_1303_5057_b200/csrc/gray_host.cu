@@ -30,7 +30,7 @@ int gray_integrate_host(const void* x_in_host, const void* k_in_host, void* x_ou
   using namespace gray;
   if (prec != GRAY_F32 && prec != GRAY_F64) { set_error("bad precision"); return GRAY_ERR_ARG; }
   if (!params) { set_error("params is NULL"); return GRAY_ERR_ARG; }
-  if (counters_host) *counters_host = gray_counters{0, 0, 0, 0};
+  if (counters_host) *counters_host = gray_counters{0, 0, 0, 0, 0};
   if (n == 0) return GRAY_OK;
   if (!x_in_host || !k_in_host || !x_out_host || !k_out_host || !status_host || !steps_host) { set_error("NULL host buffer"); return GRAY_ERR_ARG; }
   if (chunk == 0) { set_error("chunk must be positive"); return GRAY_ERR_ARG; }
@@ -42,8 +42,8 @@ int gray_integrate_host(const void* x_in_host, const void* k_in_host, void* x_ou
   const size_t vec = (prec == GRAY_F32 ? 16 : 32);
   Slot slot[2];
   char* base = (char*)scratch_dev;
-  unsigned long long* pinned = nullptr;   // 2 x 4 counters; pinned so the copies back stay asynchronous
-  GRAY_CUDA(cudaHostAlloc(&pinned, 8 * sizeof(unsigned long long), cudaHostAllocDefault));
+  unsigned long long* pinned = nullptr;   // 2 x 5 counters; pinned so the copies back stay asynchronous
+  GRAY_CUDA(cudaHostAlloc(&pinned, 10 * sizeof(unsigned long long), cudaHostAllocDefault));
   for (int s = 0; s < 2; ++s) {
     char* p = base + s * slot_bytes(chunk, prec);
     slot[s].x = p; p += align256(chunk * vec);
@@ -51,16 +51,17 @@ int gray_integrate_host(const void* x_in_host, const void* k_in_host, void* x_ou
     slot[s].steps = (uint32_t*)p; p += align256(chunk * 4);
     slot[s].status = (uint8_t*)p; p += align256(chunk);
     slot[s].ws = (Workspace*)p;
-    slot[s].c = pinned + 4 * s;
+    slot[s].c = pinned + 5 * s;
     GRAY_CUDA(cudaStreamCreateWithFlags(&slot[s].stream, cudaStreamNonBlocking));
   }
   int rc = GRAY_OK;
-  gray_counters total = {0, 0, 0, 0};
+  gray_counters total = {0, 0, 0, 0, 0};
   uint64_t done_chunks = 0;
   auto drain = [&](int s) -> int {   // wait for the chunk in flight on slot s and add its counters
     GRAY_CUDA(cudaStreamSynchronize(slot[s].stream));
     total.photon_steps += slot[s].c[0]; total.issued_steps += slot[s].c[1];
     total.photons_done += slot[s].c[2]; total.photons_live += slot[s].c[3];
+    total.fallback_steps += slot[s].c[4];
     return GRAY_OK;
   };
   for (uint64_t lo = 0; lo < n && rc == GRAY_OK; lo += chunk, ++done_chunks) {
@@ -84,7 +85,7 @@ int gray_integrate_host(const void* x_in_host, const void* k_in_host, void* x_ou
     if (e == cudaSuccess) e = cudaMemcpyAsync((char*)k_out_host + lo * vec, S.k, m * vec, cudaMemcpyDeviceToHost, S.stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(status_host + lo, S.status, m, cudaMemcpyDeviceToHost, S.stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(steps_host + lo, S.steps, m * 4, cudaMemcpyDeviceToHost, S.stream);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(S.c, &S.ws->photon_steps, 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, S.stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(S.c, &S.ws->photon_steps, 5 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, S.stream);
     if (e != cudaSuccess) { rc = cuda_fail(e, "gray_integrate_host: copy out"); break; }
   }
   const uint64_t in_flight = done_chunks < 2 ? done_chunks : 2;

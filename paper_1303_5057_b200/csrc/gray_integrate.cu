@@ -48,7 +48,7 @@ __device__ __forceinline__ unsigned long long warp_sum(unsigned long long v) {
   return v;
 }
 
-template <typename V, int RULE, int SCHED, bool FROZEN>
+template <typename V, int RULE, int SCHED, bool FROZEN, bool XI>
 __global__ void __launch_bounds__(kBlock, Tune<V>::min_blocks)
 integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
   using S = typename VT<V>::S;
@@ -65,7 +65,7 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
   bool have[N];
   bool exhausted = (SCHED == GRAY_SCHED_STATIC);
   unsigned long long c_steps = 0;
-  unsigned int c_done = 0, c_live = 0, c_iter = 0;
+  unsigned int c_done = 0, c_live = 0, c_iter = 0, c_fallback = 0;
 #pragma unroll
   for (int i = 0; i < 8; ++i) { y[i] = K.one; comp[i] = K.zero; }
 #pragma unroll
@@ -162,7 +162,12 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
       if (any) {
         const V dl = step_size<V, RULE>(K, y[1], y[5], y[6], y[7]);
         if (!FROZEN) {
-          rk4_step(K, y, comp, dl);
+          bool rej[N];
+          rk4_step<XI>(K, y, comp, dl, rej);
+          if (XI) {
+#pragma unroll
+            for (int l = 0; l < N; ++l) c_fallback += (rej[l] && have[l]) ? 1u : 0u;
+          }
           const V z = nonfinite_probe(K, y);
           const V r = vadd(y[1], K.rp);
           // Bookkeeping.  Common case first, with one branch for the whole thread: every slot's theta still in
@@ -197,7 +202,8 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
           V w[8], wc[8];
 #pragma unroll
           for (int i = 0; i < 8; ++i) { w[i] = y[i]; wc[i] = comp[i]; }
-          rk4_step(K, w, wc, dl);
+          bool rej[N];
+          rk4_step<false>(K, w, wc, dl, rej);
           const V z = nonfinite_probe(K, w);
           const V r = vadd(w[1], K.rp);
           S th[N], ph[N], kh[N], c2[N], c6[N];
@@ -240,17 +246,19 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
   c_steps = warp_sum(c_steps);
   const unsigned long long done = warp_sum((unsigned long long)c_done);
   const unsigned long long live = warp_sum((unsigned long long)c_live);
+  const unsigned long long fb = XI ? warp_sum((unsigned long long)c_fallback) : 0ull;
   if (lane == 0) {
     if (c_steps) atomicAdd(&A.ws->photon_steps, c_steps);
     if (c_iter) atomicAdd(&A.ws->issued_steps, (unsigned long long)(32 * N) * c_iter);
     if (done) atomicAdd(&A.ws->photons_done, done);
     if (live) atomicAdd(&A.ws->photons_live, live);
+    if (XI && fb) atomicAdd(&A.ws->fallback_steps, fb);
   }
 }
 
-template <typename V, int RULE, int SCHED, bool FROZEN>
+template <typename V, int RULE, int SCHED, bool FROZEN, bool XI>
 static int launch(const IntegrateArgs<V>& A, cudaStream_t stream) {
-  auto kern = integrate_kernel<V, RULE, SCHED, FROZEN>;
+  auto kern = integrate_kernel<V, RULE, SCHED, FROZEN, XI>;
   constexpr unsigned long long per_block = (unsigned long long)kBlock * VT<V>::N;
   unsigned long long blocks_needed = (A.n + per_block - 1) / per_block;
   unsigned int grid;
@@ -271,7 +279,8 @@ static int launch(const IntegrateArgs<V>& A, cudaStream_t stream) {
 
 template <typename V, int RULE, int SCHED>
 static int dispatch_frozen(const IntegrateArgs<V>& A, bool frozen, cudaStream_t s) {
-  return frozen ? launch<V, RULE, SCHED, true>(A, s) : launch<V, RULE, SCHED, false>(A, s);
+  if (frozen) return launch<V, RULE, SCHED, true, false>(A, s);
+  return A.K.xi_eps > 0 ? launch<V, RULE, SCHED, false, true>(A, s) : launch<V, RULE, SCHED, false, false>(A, s);
 }
 template <typename V, int RULE>
 static int dispatch_sched(const IntegrateArgs<V>& A, int sched, bool frozen, cudaStream_t s) {
@@ -293,7 +302,7 @@ static int integrate(const gray_state* st, uint64_t n, uint32_t max_steps, const
   A.refill_interval = p->refill_interval > 0 ? p->refill_interval : 8;
   const double a = st->a, rh = 1.0 + sqrt(1.0 - a * a);
   A.K = make_consts<V>(a, p->h, p->r_capture_factor > 0.0 ? p->r_capture_factor * rh : rh + p->horizon_delta,
-                       p->r_escape_factor * st->r_obs);
+                       p->r_escape_factor * st->r_obs, p->xi_epsilon);
   A.ws = ws;
   const bool frozen = p->frozen != 0;
   return p->rule == GRAY_STEP_EQ2 ? dispatch_sched<V, GRAY_STEP_EQ2>(A, p->schedule, frozen, stream)
@@ -314,6 +323,8 @@ int gray_integrate(gray_state* state, uint64_t n_photons, uint32_t max_steps, co
   if (params->rule != GRAY_STEP_REL && params->rule != GRAY_STEP_EQ2) { set_error("bad step rule %d", params->rule); return GRAY_ERR_ARG; }
   if (params->schedule != GRAY_SCHED_REFILL && params->schedule != GRAY_SCHED_STATIC) { set_error("bad schedule %d", params->schedule); return GRAY_ERR_ARG; }
   if (params->refill_interval < 0) { set_error("refill_interval must be >= 0"); return GRAY_ERR_ARG; }
+  if (!(params->xi_epsilon >= 0.0)) { set_error("xi_epsilon must be >= 0"); return GRAY_ERR_DOMAIN; }
+  if (params->xi_epsilon > 0.0 && params->frozen) { set_error("xi_epsilon > 0 is not available together with frozen"); return GRAY_ERR_UNSUPPORTED; }
   if (params->photons_per_thread < 0 || params->photons_per_thread > 2) { set_error("photons_per_thread must be 0 (default), 1 or 2"); return GRAY_ERR_ARG; }
   if (params->photons_per_thread == 2 && state->prec != GRAY_F32) { set_error("photons_per_thread = 2 (packed FP32 instructions) needs GRAY_F32"); return GRAY_ERR_UNSUPPORTED; }
   if (!(params->h > 0.0) || !(params->r_escape_factor > 0.0) || params->r_capture_factor < 0.0 ||
@@ -339,13 +350,14 @@ int gray_integrate_counters(const void* workspace_dev, gray_counters* counters_h
   if (rc) return rc;
   cudaStream_t stream = (cudaStream_t)cuda_stream;
   const Workspace* ws = (const Workspace*)workspace_dev;
-  unsigned long long c[4];
+  unsigned long long c[5];
   GRAY_CUDA(cudaMemcpyAsync(c, &ws->photon_steps, sizeof c, cudaMemcpyDeviceToHost, stream));
   GRAY_CUDA(cudaStreamSynchronize(stream));
   counters_host->photon_steps = c[0];
   counters_host->issued_steps = c[1];
   counters_host->photons_done = c[2];
   counters_host->photons_live = c[3];
+  counters_host->fallback_steps = c[4];
   return GRAY_OK;
 }
 

@@ -17,7 +17,8 @@ struct Workspace {
   unsigned long long issued_steps;
   unsigned long long photons_done;
   unsigned long long photons_live;
-  unsigned long long pad1[12];
+  unsigned long long fallback_steps;
+  unsigned long long pad1[11];
   unsigned long long counts[4];           // gray_classify: photons per status
   unsigned long long sum_col, sum_row;    // gray_shadow_edge: sums of captured pixel indices
   unsigned int min_col, max_col;          //                   extreme captured columns

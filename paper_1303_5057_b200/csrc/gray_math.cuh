@@ -45,14 +45,15 @@ struct Consts {
   V a, na, a2, na2, twoa2, n2a2, n2a;     // a, -a, a^2, -a^2, 2a^2, -2a^2, -2a
   V rp, rpm, rpm1;                        // r_+ (the horizon r_bh of P:75), r_+ - r_-, r_+ - 1
   V nh;                                   // -h (step parameter, the paper's Delta)
-  V zero, one, two, m2, half, nhalf, sixth;
+  V zero, one, mone, two, m2, half, nhalf, sixth, ninth;
   // sin / cos (float builds): quadrant reduction and minimax polynomials, see sincos_v
   V two_over_pi, magic, npio2_hi, npio2_lo, s1, s2, s3, c1, c2, c3, c4;
   S r_cap, r_esc;                         // termination radii
+  S xi_eps;                               // epsilon of the xi monitor (paper eq. 4); 0 = off
 };
 
 template <typename V>
-__host__ inline Consts<V> make_consts(double a, double h, double r_cap, double r_esc) {
+__host__ inline Consts<V> make_consts(double a, double h, double r_cap, double r_esc, double xi_eps) {
   using S = typename VT<V>::S;
   Consts<V> K;
   auto B = [](double v) { V r; S s = (S)v; S* p = (S*)&r; for (int i = 0; i < VT<V>::N; ++i) p[i] = s; return r; };
@@ -62,6 +63,7 @@ __host__ inline Consts<V> make_consts(double a, double h, double r_cap, double r
   K.rp = B(1.0 + root); K.rpm = B(2.0 * root); K.rpm1 = B(root);
   K.nh = B(-h);
   K.zero = B(0); K.one = B(1); K.two = B(2); K.m2 = B(-2); K.half = B(0.5); K.nhalf = B(-0.5); K.sixth = B(1.0 / 6.0);
+  K.mone = B(-1); K.ninth = B(1.0 / 9.0); K.xi_eps = (S)xi_eps;
   K.two_over_pi = B(0.636619772); K.magic = B(12582912.0);
   K.npio2_hi = B(-1.57079637050628662109375); K.npio2_lo = B(4.371139000186241e-08);
   K.s1 = B(-1.666666418e-01); K.s2 = B(8.332700469e-03); K.s3 = B(-1.957778732e-04);
@@ -177,17 +179,64 @@ GRAY_DEV V step_size(const Consts<V>& K, V d, V kr, V kh, V kp) {
   return vmax(d1, d2);
 }
 
-// ---- one classical RK4 step (P:75) of y = (t, d, th, phi, k^t, k^r, k^th, k^phi) -------------------
-// `comp` carries, for the float builds, the rounding error of each state update into the next one
-// (compensated summation): y + comp is the state to roughly twice the working precision.
+// ---- state update y <- y + scale * rate --------------------------------------------------------------
+// `comp` carries, for the float builds, the rounding error of each update into the next one (compensated
+// summation): y + comp is the state to roughly twice the working precision.
 template <typename V>
-GRAY_DEV void rk4_step(const Consts<V>& K, V y[8], V comp[8], V dl) {
-  V acc[8], w[8], f[4];
+GRAY_DEV void advance_state(const V y[8], const V comp[8], V scale, const V rate[8], V yn[8], V cn[8]) {
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    if (sizeof(typename VT<V>::S) == 4 && ((GRAY_COMP_MASK >> i) & 1)) {
+      const V inc = vfma(scale, rate[i], comp[i]);
+      const V s = vadd(y[i], inc);
+      cn[i] = vsub(inc, vsub(s, y[i]));        // Fast2Sum: exact whenever |y| >= |inc|
+      yn[i] = s;
+    } else {
+      yn[i] = vfma(scale, rate[i], y[i]);
+      cn[i] = comp[i];
+    }
+  }
+}
+
+// ---- the paper's xi (eq. 4): N = g_mu_nu k^mu k^nu and D = g_tt (k^t)^2, xi + 1 = N / D ---------------
+//   N = -(k^t)^2 + (2r/Sigma) u^2 + Sigma ((k^r)^2/Delta + (k^th)^2) + rho s^2 (k^phi)^2,  D = (2r/Sigma - 1) (k^t)^2
+template <typename V>
+GRAY_DEV void null_norm(const Consts<V>& K, const V y[8], V& Nn, V& Dn) {
+  V s, c;
+  sincos_v(K, y[2], s, c);
+  const V d = y[1], kt = y[4], kr = y[5], kh = y[6], kp = y[7];
+  const V r = vadd(d, K.rp);
+  const V r2 = vmul(r, r);
+  const V Sg = vfma(K.a2, vmul(c, c), r2);
+  const V rho = vadd(r2, K.a2);
+  const V Dl = vmul(d, vadd(d, K.rpm));
+  const V iS = vrcp(Sg), iD = vrcp(Dl);
+  const V s2 = vmul(s, s);
+  const V u = vfma(vmul(K.na, s2), kp, kt);
+  const V riS = vmul(r, iS);
+  const V kt2 = vmul(kt, kt);
+  const V B = vfma(vmul(kr, iD), kr, vmul(kh, kh));
+  const V n1 = vfma(K.two, vmul(riS, vmul(u, u)), vmul(Sg, B));
+  const V n2 = vfma(vmul(rho, vmul(s2, kp)), kp, n1);
+  Nn = vfma(vneg(kt), kt, n2);
+  Dn = vmul(vfma(K.two, riS, K.mone), kt2);
+}
+
+// ---- one classical RK4 step (P:75) of y = (t, d, th, phi, k^t, k^r, k^th, k^phi) -------------------
+// XI: the paper's production pole treatment: if the state the RK4 step produced has |xi + 1| > epsilon
+// (or a non-finite xi), the step is re-integrated from the old state as one forward Euler step of dlambda / 9,
+// which is not tested itself.  rejected[l] reports it per photon.
+template <bool XI, typename V>
+GRAY_DEV void rk4_step(const Consts<V>& K, V y[8], V comp[8], V dl, bool rejected[VT<V>::N]) {
+  using S = typename VT<V>::S;
+  constexpr int N = VT<V>::N;
+  V acc[8], w[8], f[4], f1[4];
   const V hdl = vmul(K.half, dl);
   // stage 1
   geodesic_accel<false>(K, y[1], y[2], y[4], y[5], y[6], y[7], (const V*)nullptr, f);
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
+    f1[i] = f[i];
     acc[i] = y[4 + i];
     acc[4 + i] = f[i];
     w[i] = vfma(hdl, y[4 + i], y[i]);
@@ -211,18 +260,38 @@ GRAY_DEV void rk4_step(const Consts<V>& K, V y[8], V comp[8], V dl) {
 #pragma unroll
   for (int i = 0; i < 4; ++i) acc[i] = vadd(acc[i], w[4 + i]);
   geodesic_accel<true>(K, w[1], w[2], w[4], w[5], w[6], w[7], acc + 4, acc + 4);
-  const V dl6 = vmul(K.sixth, dl);
+  V yn[8], cn[8];
+  advance_state(y, comp, vmul(K.sixth, dl), acc, yn, cn);
 #pragma unroll
-  for (int i = 0; i < 8; ++i) {
-    if (sizeof(typename VT<V>::S) == 4 && ((GRAY_COMP_MASK >> i) & 1)) {
-      const V inc = vfma(dl6, acc[i], comp[i]);
-      const V s = vadd(y[i], inc);
-      comp[i] = vsub(inc, vsub(s, y[i]));      // Fast2Sum: exact whenever |y| >= |inc|
-      y[i] = s;
-    } else {
-      y[i] = vfma(dl6, acc[i], y[i]);
+  for (int l = 0; l < N; ++l) rejected[l] = false;
+  if (XI) {
+    V Nn, Dn;
+    null_norm(K, yn, Nn, Dn);
+    S nn[N], dn[N];
+    vunpack(Nn, nn); vunpack(Dn, dn);
+    bool any = false;
+#pragma unroll
+    for (int l = 0; l < N; ++l) {
+      rejected[l] = !(sabs(nn[l]) <= vmul(K.xi_eps, sabs(dn[l])));
+      any |= rejected[l];
+    }
+    if (any) {
+      V rate[8], ye[8], ce[8];
+#pragma unroll
+      for (int i = 0; i < 4; ++i) { rate[i] = y[4 + i]; rate[4 + i] = f1[i]; }
+      advance_state(y, comp, vmul(K.ninth, dl), rate, ye, ce);
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        S a[N], b[N], ca[N], cb[N];
+        vunpack(yn[i], a); vunpack(ye[i], b); vunpack(cn[i], ca); vunpack(ce[i], cb);
+#pragma unroll
+        for (int l = 0; l < N; ++l) { a[l] = rejected[l] ? b[l] : a[l]; ca[l] = rejected[l] ? cb[l] : ca[l]; }
+        vpack(yn[i], a); vpack(cn[i], ca);
+      }
     }
   }
+#pragma unroll
+  for (int i = 0; i < 8; ++i) { y[i] = yn[i]; comp[i] = cn[i]; }
 }
 
 // pi and 2 pi minus x with pi split in two parts of the working precision

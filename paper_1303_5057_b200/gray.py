@@ -33,12 +33,12 @@ class _StepParams(C.Structure):
     _fields_ = [("h", C.c_double), ("r_capture_factor", C.c_double), ("horizon_delta", C.c_double),
                 ("r_escape_factor", C.c_double), ("rule", C.c_int32), ("schedule", C.c_int32),
                 ("refill_interval", C.c_int32), ("frozen", C.c_int32), ("photons_per_thread", C.c_int32),
-                ("reserved", C.c_int32)]
+                ("reserved", C.c_int32), ("xi_epsilon", C.c_double)]
 
 
 class _Counters(C.Structure):
     _fields_ = [("photon_steps", C.c_uint64), ("issued_steps", C.c_uint64), ("photons_done", C.c_uint64),
-                ("photons_live", C.c_uint64)]
+                ("photons_live", C.c_uint64), ("fallback_steps", C.c_uint64)]
 
 
 class _ShadowStats(C.Structure):
@@ -100,9 +100,9 @@ class StepParams:
     """gray_step_params (include/gray.h).  Defaults: the BASELINE configs' h, capture and escape radii."""
 
     def __init__(self, h=1.0 / 32, r_capture_factor=1.01, horizon_delta=1e-6, r_escape_factor=1.01, rule=STEP_EQ2,
-                 schedule=SCHED_REFILL, refill_interval=0, frozen=False, photons_per_thread=0):
+                 schedule=SCHED_REFILL, refill_interval=0, frozen=False, photons_per_thread=0, xi_epsilon=0.0):
         self.c = _StepParams(h, r_capture_factor, horizon_delta, r_escape_factor, rule, schedule, refill_interval,
-                             int(bool(frozen)), photons_per_thread, 0)
+                             int(bool(frozen)), photons_per_thread, 0, xi_epsilon)
 
 
 class PhotonBatch:
@@ -155,7 +155,7 @@ def gray_integrate_counters(batch):
     c = _Counters()
     _check(lib().gray_integrate_counters(_ptr(batch.workspace), C.byref(c), _stream()))
     return dict(photon_steps=c.photon_steps, issued_steps=c.issued_steps, photons_done=c.photons_done,
-                photons_live=c.photons_live)
+                photons_live=c.photons_live, fallback_steps=c.fallback_steps)
 
 
 def gray_classify(batch, capture_map=None):
@@ -193,7 +193,7 @@ def gray_integrate_host(x_in, k_in, x_out, k_out, status, steps, a, r_obs, max_s
                                      prec, a, r_obs, max_steps, C.byref(params.c), chunk, _ptr(scratch),
                                      scratch.numel(), C.byref(c)))
     return dict(photon_steps=c.photon_steps, issued_steps=c.issued_steps, photons_done=c.photons_done,
-                photons_live=c.photons_live)
+                photons_live=c.photons_live, fallback_steps=c.fallback_steps)
 
 
 def gray_fma_peak(prec=GRAY_F32, iters=4096):

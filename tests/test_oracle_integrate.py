@@ -218,3 +218,27 @@ def test_op_tally_is_stable_and_plausible():
     assert 600 < flops < 900
     te = o.op_tally(a, y, 1 / 32, o.STEP_EQ2)
     assert te["div"] > t["div"] and te["sqrt"] == 1
+
+
+def test_pole_treatment_xi_monitor_cures_the_pole_failures():
+    # NEXT-1.  Pin: the exact radial-potential classifier (independent of any integrator).  Rays of the
+    # pixel column next to the spin axis of a face-on-ish image (a = 0.8, i = 5 deg, 1024 x 1024 over +-10 M),
+    # well inside the shadow: plain RK4 "kicks" some of them "back to infinity" at the pole; with the xi
+    # monitor of eq. (4) at epsilon = 1e-3 every one is captured, as the paper reports for its own
+    # 3e8 trajectories.
+    a, inc, W, nx = 0.8, 5.0, 10.0, 1024
+    cols, rows = np.arange(511, 514), np.arange(284, 308)
+    idx = (cols[None, :] + nx * rows[:, None]).ravel().astype(np.uint64)
+    plain = o.trace(a, 1000.0, inc, W, nx, nx, idx=idx, rule=o.STEP_EQ2, threads=8)
+    inv = np.array([o.invariants(a, v) for v in plain["y0"]])
+    exact = np.array([cf.captured_exact(a, L / E, Q / E ** 2) for E, L, Q, _ in inv])
+    assert exact.all()                                                  # every ray of the strip is inside the shadow
+    assert np.sum(plain["status"] == o.ESCAPED) >= 3                    # the failure
+    cured = o.trace(a, 1000.0, inc, W, nx, nx, idx=idx, rule=o.STEP_EQ2, threads=8, xi_eps=1e-3)
+    assert np.all(cured["status"] == o.CAPTURED)                        # the cure
+    # away from the pole the monitor never fires: identical results
+    idx2 = (np.arange(200, 216)[None, :] + nx * np.arange(500, 504)[:, None]).ravel().astype(np.uint64)
+    p2 = o.trace(a, 1000.0, inc, W, nx, nx, idx=idx2, rule=o.STEP_EQ2)
+    c2 = o.trace(a, 1000.0, inc, W, nx, nx, idx=idx2, rule=o.STEP_EQ2, xi_eps=1e-3)
+    esc = p2["status"] == o.ESCAPED
+    assert esc.any() and np.array_equal(p2["y"][esc], c2["y"][esc]) and np.array_equal(p2["steps"][esc], c2["steps"][esc])
