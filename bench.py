@@ -50,6 +50,7 @@ def parse():
     ap.add_argument("--schedule", default="refill", choices=["refill", "static"])
     ap.add_argument("--refill-interval", type=int, default=0)
     ap.add_argument("--photons-per-thread", type=int, default=0, help="0 = library default (2 for f32: packed FFMA2), 1, 2")
+    ap.add_argument("--xi-eps", type=float, default=0.0, help="epsilon of the paper's xi monitor (P:107); 0 = off")
     ap.add_argument("--e2e-log2n", type=int, default=-1, help="photons per GPU of the host-buffer run (default min(log2n, 26))")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -107,7 +108,7 @@ def workload_config(args, world):
     return {"workload": f"C4-{args.case}: 2^{args.log2n} photons/GPU, Kerr a={c4['a']}, i={c4['inc_deg']} deg, seeded random "
                         f"pixels over +-{c4['half_width']} M at r_obs={wl.R_OBS:.0f} M, RK4 h=1/32, rule={args.rule}",
             "photons_per_gpu": 2 ** args.log2n, "photons_total": world * 2 ** args.log2n, "precision": args.prec,
-            "step_rule": args.rule, "case": args.case, "schedule": args.schedule, "max_steps": wl.MAX_STEPS if args.case == "realistic" else c4["peak_steps"],
+            "step_rule": args.rule, "case": args.case, "schedule": args.schedule, "xi_epsilon": args.xi_eps, "max_steps": wl.MAX_STEPS if args.case == "realistic" else c4["peak_steps"],
             "seed": c4["seed"], "parallelism": f"photon-range sharding x{world}, no collective on the data path",
             "l2": "state (37 B/photon) far larger than the 126 MB L2; no flush needed"}
 
@@ -182,7 +183,7 @@ def run_gray(args):
     params = g.StepParams(h=wl.H, r_capture_factor=wl.R_CAPTURE_FACTOR, r_escape_factor=wl.R_ESCAPE_FACTOR, rule=rule,
                           schedule=g.SCHED_REFILL if args.schedule == "refill" else g.SCHED_STATIC,
                           refill_interval=args.refill_interval, frozen=peak_case,
-                          photons_per_thread=args.photons_per_thread)
+                          photons_per_thread=args.photons_per_thread, xi_epsilon=args.xi_eps)
     batch = g.PhotonBatch(n, prec, device=dev)
     p0 = rank * n                                   # weak scaling: every rank its own photon range
 
