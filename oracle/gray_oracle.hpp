@@ -24,6 +24,8 @@
 //                           classifier (Kerr), Schwarzschild deflection
 //                           quadrature, reflection / spin-flip symmetries,
 //                           the face-on critical radius next to P:91's value
+//   pole treatment        : advance() with xi_eps > 0 (paper P:103-107) against the
+//                           exact classifier on rays next to the spin axis
 //   shadow statistics     : Bardeen closed-form curve (area, alpha extent, D,
 //                           <R>, A), an exact synthetic disc, paper eqs. 11-14
 // Parity unpinned (GPU-vs-oracle only): the final state of CAPTURED rays at
