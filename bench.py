@@ -282,6 +282,13 @@ def run_gray(args):
     achieved = flops * counted / (kern_ms * 1e-3) / 1e12
     peak = PEAK_TFLOPS[args.prec]
     fma_peak = g.gray_fma_peak(prec, 8192) / 1e12
+    # Achievable ceiling of the packed fp32 kernel: the FP32 pipe retires the
+    # integrator's mix of FMUL2 / FFMA2 / FADD2 with changing register operands at this fraction of its lane rate
+    mix = None
+    if args.prec == "f32" and args.photons_per_thread != 1:
+        lane_peak = 148 * 128 * 1.965e9
+        mix = {"ffma2_invariant_operands": g.gray_packed_peak(0) / lane_peak, "ffma2_three_register_pairs": g.gray_packed_peak(1) / lane_peak,
+               "integrator_mix": g.gray_packed_peak(2) / lane_peak}
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                 "traffic": (NCU_DRAM_BYTES_PER_PHOTON * n) if (NCU_DRAM_BYTES_PER_PHOTON and args.prec == "f32") else None,
                 "traffic_source": "ncu dram bytes per photon at 2^22 photons x photons of this launch",
@@ -290,6 +297,8 @@ def run_gray(args):
                 "peak_source": "148 SMs x %d lanes x 2 x 1.965 GHz (DESIGN.md)" % (128 if args.prec == "f32" else 64),
                 "fma_microbench_tflops": fma_peak, "frac_of_fma_microbench": achieved / fma_peak,
                 "lane_efficiency": tot_steps / tot_issued if tot_issued else None,
+                "packed_pipe_fraction_measured": mix,
+                "frac_of_achievable": (achieved / peak) / (mix["integrator_mix"] * 787.0 / 792.0) if mix else None,
                 "hbm_algorithmic_bytes_per_launch": n * (2 * (32 if args.prec == "f32" else 64) + 10)}
     out = {"metric": "photon-steps/s", "value": value, "unit": "photon-steps/s", "n_gpus": world, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",

@@ -203,6 +203,17 @@ GRAY_API int gray_integrate_host(const void* x_in_host, const void* k_in_host, v
  * on every SM, times them with CUDA events on the stream, returns FLOP/s (FMA = 2).  Synchronises.  */
 GRAY_API int gray_fma_peak(int32_t prec, int32_t iters, double* flops_per_s_host, void* cuda_stream);
 
+/* Packed FP32 (FFMA2 / FMUL2 / FADD2, the instructions of the GRAY_F32 integrator) register-only microbenchmark,
+ * 16 warps per SM like the integrator: the rate at which the FP32 pipe retires packed instructions depends on how
+ * many distinct register pairs an instruction reads (register-file bandwidth), which bounds the integrator below
+ * the FFMA peak.
+ *   mix 0  FFMA2 x <- x * m + c with loop-invariant m, c
+ *   mix 1  FFMA2 reading three different, changing register pairs
+ *   mix 2  the integrator's instruction mix: 50 % FMUL2, 37.5 % FFMA2 (three pairs), 12.5 % FADD2
+ * Returns fp32 lane-operations per second (one FFMA2 = 2 per thread; multiply by 2 for FMA flops of mix 0 / 1).
+ * Synchronises.                                                                                             */
+GRAY_API int gray_packed_peak(int32_t mix, int32_t iters, double* lane_ops_per_s_host, void* cuda_stream);
+
 /* Device facts used by the benchmark: SM count and SM clock (kHz) reported by the runtime.         */
 GRAY_API int gray_device_info(int32_t* sm_count_host, int32_t* sm_clock_khz_host);
 

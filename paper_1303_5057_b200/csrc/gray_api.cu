@@ -99,6 +99,76 @@ static int fma_peak(int iters, double* out, cudaStream_t stream) {
   return GRAY_OK;
 }
 
+// Packed FP32 (FFMA2 / FMUL2 / FADD2) throughput for three operand patterns (gray_packed_peak in gray.h).
+typedef unsigned long long u64_t;
+__device__ __forceinline__ u64_t p_fma2(u64_t a, u64_t b, u64_t c) { u64_t d; asm volatile("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+__device__ __forceinline__ u64_t p_mul2(u64_t a, u64_t b) { u64_t d; asm volatile("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ u64_t p_add2(u64_t a, u64_t b) { u64_t d; asm volatile("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+
+template <int MIX>
+__global__ void __launch_bounds__(128, 4) packed_peak_kernel(int iters, const u64_t* in, u64_t* sink) {
+  u64_t x[16];
+#pragma unroll
+  for (int i = 0; i < 16; ++i) x[i] = in[(threadIdx.x * 16 + i) & 1023];
+  const u64_t m = in[5], c = in[9];
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+#pragma unroll
+      for (int i = 0; i < 16; ++i) {
+        if (MIX == 0) x[i] = p_fma2(x[i], m, c);
+        if (MIX == 1) x[i] = p_fma2(x[i], x[(i + 3) & 15], x[(i + 7) & 15]);
+        if (MIX == 2) {
+          const int s = (i + r) & 7;
+          if (s < 4) x[i] = p_mul2(x[i], x[(i + 5) & 15]);
+          else if (s < 7) x[i] = p_fma2(x[i], x[(i + 3) & 15], x[(i + 9) & 15]);
+          else x[i] = p_add2(x[i], x[(i + 1) & 15]);
+        }
+      }
+    }
+  }
+  u64_t a = 0;
+#pragma unroll
+  for (int i = 0; i < 16; ++i) a ^= x[i];
+  if (a == 12345ull) sink[0] = a;   // never true; keeps the loop alive
+}
+
+template <int MIX>
+static int packed_peak(int iters, double* out, cudaStream_t stream) {
+  const int sms = sm_count();
+  if (sms <= 0) { set_error("no CUDA device"); return GRAY_ERR_CUDA; }
+  u64_t host[1024];
+  for (int i = 0; i < 1024; ++i) {
+    const float lo = 1.0f + 1e-4f * (float)(i % 7), hi = 1.0f - 1e-4f * (float)(i % 5);
+    unsigned ul, uh;
+    memcpy(&ul, &lo, 4); memcpy(&uh, &hi, 4);
+    host[i] = ((u64_t)uh << 32) | ul;
+  }
+  u64_t* buf = nullptr;
+  GRAY_CUDA(cudaMalloc(&buf, sizeof host + 8));
+  cudaError_t e = cudaMemcpyAsync(buf, host, sizeof host, cudaMemcpyHostToDevice, stream);
+  if (e != cudaSuccess) { cudaFree(buf); return cuda_fail(e, "cudaMemcpyAsync"); }
+  const int blocks = sms * 4, threads = 128;      // 16 warps per SM, as the integrator has
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  packed_peak_kernel<MIX><<<blocks, threads, 0, stream>>>(iters / 8 + 1, buf, buf + 1024);
+  float best = 1e30f;
+  for (int rep = 0; rep < 3; ++rep) {
+    cudaEventRecord(e0, stream);
+    packed_peak_kernel<MIX><<<blocks, threads, 0, stream>>>(iters, buf, buf + 1024);
+    cudaEventRecord(e1, stream);
+    e = cudaEventSynchronize(e1);
+    if (e != cudaSuccess) { cudaFree(buf); return cuda_fail(e, "packed_peak_kernel"); }
+    float ms = 0;
+    cudaEventElapsedTime(&ms, e0, e1);
+    if (ms < best) best = ms;
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  cudaFree(buf);
+  *out = 2.0 * 64.0 * (double)iters * (double)blocks * (double)threads / (best * 1e-3);   // fp32 lane-operations / s
+  return GRAY_OK;
+}
+
 }  // namespace gray
 
 extern "C" {
@@ -124,6 +194,16 @@ int gray_fma_peak(int32_t prec, int32_t iters, double* flops_per_s_host, void* c
   if (prec == GRAY_F32) return gray::fma_peak<float>(iters, flops_per_s_host, s);
   if (prec == GRAY_F64) return gray::fma_peak<double>(iters, flops_per_s_host, s);
   gray::set_error("gray_fma_peak: bad precision");
+  return GRAY_ERR_ARG;
+}
+
+int gray_packed_peak(int32_t mix, int32_t iters, double* lane_ops_per_s_host, void* cuda_stream) {
+  if (!lane_ops_per_s_host || iters <= 0) { gray::set_error("gray_packed_peak: bad arguments"); return GRAY_ERR_ARG; }
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  if (mix == 0) return gray::packed_peak<0>(iters, lane_ops_per_s_host, s);
+  if (mix == 1) return gray::packed_peak<1>(iters, lane_ops_per_s_host, s);
+  if (mix == 2) return gray::packed_peak<2>(iters, lane_ops_per_s_host, s);
+  gray::set_error("gray_packed_peak: mix must be 0, 1 or 2");
   return GRAY_ERR_ARG;
 }
 

@@ -73,11 +73,12 @@ def lib():
         L.gray_integrate_host.argtypes = [vp, vp, vp, vp, vp, vp, u64, i32, dbl, dbl, C.c_uint32, C.POINTER(_StepParams),
                                           u64, vp, C.c_size_t, C.POINTER(_Counters)]
         L.gray_fma_peak.argtypes = [i32, i32, C.POINTER(dbl), vp]
+        L.gray_packed_peak.argtypes = [i32, i32, C.POINTER(dbl), vp]
         L.gray_device_info.argtypes = [C.POINTER(i32), C.POINTER(i32)]
         L.gray_last_error.restype = C.c_char_p
         L.gray_version.restype = C.c_char_p
         for name in ("gray_init_rays", "gray_init_rays_random", "gray_integrate", "gray_integrate_counters",
-                     "gray_classify", "gray_shadow_edge", "gray_fma_peak", "gray_device_info", "gray_integrate_host"):
+                     "gray_classify", "gray_shadow_edge", "gray_fma_peak", "gray_packed_peak", "gray_device_info", "gray_integrate_host"):
             getattr(L, name).restype = C.c_int
         _LIB = L
     return _LIB
@@ -199,6 +200,13 @@ def gray_integrate_host(x_in, k_in, x_out, k_out, status, steps, a, r_obs, max_s
 def gray_fma_peak(prec=GRAY_F32, iters=4096):
     v = C.c_double()
     _check(lib().gray_fma_peak(prec, iters, C.byref(v), _stream()))
+    return v.value
+
+
+def gray_packed_peak(mix, iters=2048):
+    """fp32 lane-operations/s of the packed-instruction microbenchmark (include/gray.h)."""
+    v = C.c_double()
+    _check(lib().gray_packed_peak(mix, iters, C.byref(v), _stream()))
     return v.value
 
 
