@@ -59,7 +59,8 @@ typedef enum { GRAY_F32 = 0, GRAY_F64 = 1 } gray_prec;
  *                  paper eq. (2), with its Delta := h ~ 1/32                          */
 typedef enum { GRAY_STEP_REL = 0, GRAY_STEP_EQ2 = 1 } gray_step_rule;
 
-typedef enum { GRAY_LIVE = 0, GRAY_CAPTURED = 1, GRAY_ESCAPED = 2, GRAY_BAD = 3 } gray_ray_status;
+typedef enum { GRAY_LIVE = 0, GRAY_CAPTURED = 1, GRAY_ESCAPED = 2, GRAY_BAD = 3,
+               GRAY_EQUATOR = 4 /* reached theta = pi/2 (stop_at_equator only) */ } gray_ray_status;
 
 /* How photons are mapped to threads by gray_integrate.
  *   GRAY_SCHED_REFILL  persistent warps; a lane whose photon has terminated fetches the next live
@@ -124,7 +125,15 @@ typedef struct {
                                 advanced together by the packed sm_100a FP32 instructions (FFMA2 /
                                 FMUL2 / FADD2, GRAY_F32 only); 1 = one photon per thread, scalar
                                 instructions.  Per-photon results are bit-identical for 1 and 2.       */
-  int32_t reserved;          /* must be 0                                                             */
+  int32_t stop_at_equator;   /* != 0: the paper's grid-projection workload: a photon stops when it
+                                first reaches the equatorial plane.  A step crosses the plane if its start lies
+                                on one side (theta <= pi/2 is the upper side) and its end strictly on the other;
+                                unless that end state is BAD or CAPTURED, the photon is then landed on the plane
+                                by two Newton iterations - ordinary, counted steps of size
+                                dlambda = -(theta - pi/2) / k^theta - and gets status GRAY_EQUATOR; the stored
+                                state is the one after the second (theta within rounding of pi/2).  Test
+                                order: BAD, CAPTURED, EQUATOR, ESCAPED.  gray_classify counts statuses 0-3 only.
+                                Not available together with `frozen`.                                 */
   double xi_epsilon;         /* > 0: the paper's production pole treatment: after every RK4 step
                                 xi of eq. (4) is evaluated at the new state; if |xi + 1| > xi_epsilon (the
                                 paper's epsilon ~ 1e-3) or xi is not finite, the step is discarded and

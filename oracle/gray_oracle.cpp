@@ -84,8 +84,9 @@ void gray_oracle_remap_theta(double* y) { go::remap_theta(y); }
 
 // Integrate one ray from state y (in/out).  See gray_oracle::integrate.
 int gray_oracle_integrate(double a, double* y, double h, double r_capture, double r_escape, int rule,
-                          uint32_t max_steps, int64_t force_steps, uint32_t* steps, double xi_eps) {
-  go::StepParams sp{h, r_capture, r_escape, rule, xi_eps};
+                          uint32_t max_steps, int64_t force_steps, uint32_t* steps, double xi_eps,
+                          int stop_at_equator) {
+  go::StepParams sp{h, r_capture, r_escape, rule, xi_eps, stop_at_equator};
   return go::integrate(a, y, sp, max_steps, force_steps, steps);
 }
 
@@ -99,16 +100,18 @@ int gray_oracle_integrate(double a, double* y, double h, double r_capture, doubl
 //   force_steps   : NULL, or per ray a step count to take regardless of the tests
 //                   (< 0: normal termination)
 //   xi_eps > 0    : the paper's pole treatment (gray_oracle::advance)
+//   stop_at_equator: the grid-projection workload (gray_oracle::equator_land)
 // Outputs (any may be NULL): y0 (n x 8), y (n x 8), status (n), steps (n).
 // Rays are split statically and contiguously across n_threads std::threads.
 int gray_oracle_trace(double a, double r_obs, double inc_deg, double W, int64_t nx, int64_t ny,
                       uint64_t seed, const uint64_t* idx, uint64_t n_idx, double h, double cap_factor,
                       double esc_factor, double horizon_delta, int rule, uint32_t max_steps,
                       int init_f32, const int64_t* force_steps, int n_threads, double* y0_out,
-                      double* y_out, int32_t* status_out, uint32_t* steps_out, double xi_eps) {
+                      double* y_out, int32_t* status_out, uint32_t* steps_out, double xi_eps, int stop_at_equator) {
   if (n_threads < 1) n_threads = 1;
   double rh = go::horizon(a);
-  go::StepParams sp{h, cap_factor > 0 ? cap_factor * rh : rh + horizon_delta, esc_factor * r_obs, rule, xi_eps};
+  go::StepParams sp{h, cap_factor > 0 ? cap_factor * rh : rh + horizon_delta, esc_factor * r_obs, rule, xi_eps,
+                    stop_at_equator};
   double inc = inc_deg * kPi / 180.0;
   auto work = [&](uint64_t lo, uint64_t hi) {
     for (uint64_t j = lo; j < hi; ++j) {

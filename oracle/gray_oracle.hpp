@@ -26,17 +26,21 @@
 //                           the face-on critical radius next to P:91's value
 //   pole treatment        : advance() with xi_eps > 0 (paper P:103-107) against the
 //                           exact classifier on rays next to the spin axis
+//   equatorial projection : a = 0 line of nodes and orbit integral (phi, r at the
+//                           crossing to 2e-6); Kerr: invariants at the landed state,
+//                           reflection symmetry
 //   shadow statistics     : Bardeen closed-form curve (area, alpha extent, D,
 //                           <R>, A), an exact synthetic disc, paper eqs. 11-14
 // Parity unpinned (GPU-vs-oracle only): the final state of CAPTURED rays at
-// 1.01 r_h, and the EQ2 step rule's min() selection on individual steps.
+// 1.01 r_h, the EQ2 step rule's min() selection on individual steps, and the
+// Kerr (a != 0) equatorial crossing radius beyond the invariants above.
 #pragma once
 #include <cmath>
 #include <cstdint>
 
 namespace gray_oracle {
 
-enum Status : int { LIVE = 0, CAPTURED = 1, ESCAPED = 2, BAD = 3 };
+enum Status : int { LIVE = 0, CAPTURED = 1, ESCAPED = 2, BAD = 3, EQUATOR = 4 };
 enum StepRule : int { STEP_REL = 0, STEP_EQ2 = 1 };
 
 // ---------------------------------------------------------------- geometry
@@ -278,6 +282,7 @@ struct StepParams {
   double r_escape;     // escaped  when r >  r_escape   (1.01 r_obs)
   int rule;            // StepRule
   double xi_eps = 0.0; // > 0: the paper's production pole treatment with epsilon = xi_eps, see integrate()
+  int stop_at_equator = 0;  // != 0: the grid-projection workload, see equator_hit()
 };
 
 // Status of a state after a full step: non-finite -> BAD,
@@ -297,8 +302,8 @@ inline int classify_state(const double y[8], const StepParams& sp) {
 // the test is applied to the state an RK4 step produced; on failure that step is discarded and replaced by ONE
 // forward Euler step of dlambda/9 from the state before it, which is not tested itself; a non-finite xi fails
 // the test.  One step (RK4 or its Euler replacement) counts as one step.
-inline void advance(double a, double y[8], const StepParams& sp) {
-  double dl = step_size(a, y, sp.h, sp.rule);
+inline void advance(double a, double y[8], const StepParams& sp, const double* forced_dl = nullptr) {
+  double dl = forced_dl ? *forced_dl : step_size(a, y, sp.h, sp.rule);
   if (!(sp.xi_eps > 0.0)) { rk4_step(a, y, dl); return; }
   double y_old[8], inv[4];
   for (int i = 0; i < 8; ++i) y_old[i] = y[i];
@@ -311,11 +316,31 @@ inline void advance(double a, double y[8], const StepParams& sp) {
   }
 }
 
-// Integrate one ray until it is captured, escapes, goes non-finite or has taken
-// max_steps steps in total.  *steps is the running step counter (in/out), so a
-// call can resume an earlier one.  If force_steps >= 0 the tests are ignored and
-// exactly that many further steps are taken (the equal-step-count protocol,
-// DESIGN.md reading R11); the returned status is then that of the last state.
+// The paper's first benchmark (Fig. 3; NEXT-2 of SURVEY §8(f)): project the image-plane grid
+// onto the equatorial plane, i.e. follow each ray until it first reaches theta = pi/2.  Reading (R19):
+// a step crosses the plane if its start lies on one side (theta <= pi/2 counts as the upper side) and its end
+// strictly on the other.  The ray is then landed on the plane with two Newton iterations, each an ordinary step
+// (same scheme, counted like any step) whose size is dlambda = -(theta - pi/2) / k^theta instead of the step
+// rule; the state after the second one is the result (theta within ~1e-9 of pi/2, all eight components fourth
+// order accurate).  During the landing the termination tests are not applied.
+inline bool equator_crossed(double th_old, const double y[8]) {
+  const double half_pi = 1.57079632679489661923;
+  return th_old <= half_pi ? (y[2] > half_pi) : (y[2] < half_pi);
+}
+inline void equator_land(double a, double y[8], const StepParams& sp, uint32_t* steps) {
+  const double half_pi = 1.57079632679489661923;
+  for (int it = 0; it < 2; ++it) {
+    double dl = -(y[2] - half_pi) / y[6];
+    advance(a, y, sp, &dl);
+    ++*steps;
+  }
+}
+
+// Integrate one ray until it is captured, escapes, goes non-finite, (optionally) reaches the equatorial plane,
+// or has taken max_steps steps in total.  Test order: BAD, CAPTURED, EQUATOR, ESCAPED.  *steps is the running
+// step counter (in/out), so a call can resume an earlier one.  If force_steps >= 0 the tests are ignored and
+// exactly that many further steps are taken (the equal-step-count protocol, reading R11); the
+// returned status is then that of the last state.
 inline int integrate(double a, double y[8], const StepParams& sp, uint32_t max_steps,
                      int64_t force_steps, uint32_t* steps) {
   if (force_steps >= 0) {
@@ -328,10 +353,15 @@ inline int integrate(double a, double y[8], const StepParams& sp, uint32_t max_s
   }
   int st = LIVE;
   while (*steps < max_steps) {
+    double th_old = y[2];
     advance(a, y, sp);
     remap_theta(y);
     ++*steps;
     st = classify_state(y, sp);
+    if (sp.stop_at_equator && (st == LIVE || st == ESCAPED) && equator_crossed(th_old, y)) {
+      equator_land(a, y, sp, steps);
+      st = classify_state(y, sp) == BAD ? BAD : EQUATOR;
+    }
     if (st != LIVE) break;
   }
   return st;

@@ -9,7 +9,7 @@ import numpy as np
 
 from . import build as _build
 
-LIVE, CAPTURED, ESCAPED, BAD = 0, 1, 2, 3
+LIVE, CAPTURED, ESCAPED, BAD, EQUATOR = 0, 1, 2, 3, 4
 STEP_REL, STEP_EQ2 = 0, 1
 
 _lib = None
@@ -36,13 +36,13 @@ def lib():
         L.gray_oracle_remap_theta.argtypes = [_dp]
         L.gray_oracle_integrate.restype = C.c_int
         L.gray_oracle_integrate.argtypes = [C.c_double, _dp, C.c_double, C.c_double, C.c_double, C.c_int,
-                                            C.c_uint32, C.c_int64, C.POINTER(C.c_uint32), C.c_double]
+                                            C.c_uint32, C.c_int64, C.POINTER(C.c_uint32), C.c_double, C.c_int]
         L.gray_oracle_trace.restype = C.c_int
         L.gray_oracle_trace.argtypes = [C.c_double] * 4 + [C.c_int64, C.c_int64, C.c_uint64, C.c_void_p,
                                                             C.c_uint64, C.c_double, C.c_double, C.c_double,
                                                             C.c_double, C.c_int, C.c_uint32, C.c_int,
                                                             C.c_void_p, C.c_int, C.c_void_p, C.c_void_p,
-                                                            C.c_void_p, C.c_void_p, C.c_double]
+                                                            C.c_void_p, C.c_void_p, C.c_double, C.c_int]
         L.gray_oracle_hardware_threads.restype = C.c_int
         L.gray_oracle_shadow_stats.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_double, C.c_int32,
                                                C.c_void_p, C.c_void_p]
@@ -123,12 +123,12 @@ def remap_theta(y):
     return y
 
 
-def integrate(a, y, h, r_capture, r_escape, rule, max_steps, force_steps=-1, steps=0, xi_eps=0.0):
+def integrate(a, y, h, r_capture, r_escape, rule, max_steps, force_steps=-1, steps=0, xi_eps=0.0, stop_at_equator=False):
     """Integrate one ray; returns (y, status, steps)."""
     y = _vec(y, 8).copy()
     st = C.c_uint32(steps)
     status = lib().gray_oracle_integrate(a, y.ctypes.data_as(_dp), h, r_capture, r_escape, rule, max_steps,
-                                         force_steps, C.byref(st), xi_eps)
+                                         force_steps, C.byref(st), xi_eps, int(bool(stop_at_equator)))
     return y, status, st.value
 
 
@@ -138,7 +138,7 @@ def hardware_threads():
 
 def trace(a, r_obs, inc_deg, W, nx=0, ny=0, seed=0, idx=None, n=None, h=1.0 / 32, cap_factor=1.01,
           esc_factor=1.01, horizon_delta=1e-6, rule=STEP_EQ2, max_steps=20000, init_f32=False,
-          force_steps=None, threads=1, want_y0=True, xi_eps=0.0):
+          force_steps=None, threads=1, want_y0=True, xi_eps=0.0, stop_at_equator=False):
     """Initialise and integrate a batch of photons; see gray_oracle_trace in gray_oracle.cpp.
 
     Returns dict(y0, y, status, steps).
@@ -160,7 +160,7 @@ def trace(a, r_obs, inc_deg, W, nx=0, ny=0, seed=0, idx=None, n=None, h=1.0 / 32
                             horizon_delta, rule, max_steps, int(bool(init_f32)),
                             force_steps.ctypes.data if force_steps is not None else None, threads,
                             y0.ctypes.data if y0 is not None else None, y.ctypes.data,
-                            status.ctypes.data, steps.ctypes.data, xi_eps)
+                            status.ctypes.data, steps.ctypes.data, xi_eps, int(bool(stop_at_equator)))
     return dict(y0=y0, y=y, status=status, steps=steps)
 
 

@@ -26,6 +26,7 @@ struct IntegrateArgs {
   unsigned long long n;
   uint32_t max_steps;
   int refill_interval;
+  int stop_eq;               // gray_step_params.stop_at_equator
   Workspace* ws;
   Consts<V> K;
 };
@@ -48,7 +49,7 @@ __device__ __forceinline__ unsigned long long warp_sum(unsigned long long v) {
   return v;
 }
 
-template <typename V, int RULE, int SCHED, bool FROZEN, bool XI>
+template <typename V, int RULE, int SCHED, bool FROZEN, bool XI, bool EQ>
 __global__ void __launch_bounds__(kBlock, Tune<V>::min_blocks)
 integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
   using S = typename VT<V>::S;
@@ -62,6 +63,8 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
   unsigned long long idx[N];
   uint32_t nst[N], nst0[N], iss[N];
   int fstat[N];
+  int landing[N];            // stop_at_equator: 0 = cruising, 1 / 2 = before the first / second Newton step onto the plane
+  bool lnd = false;          // any slot of this thread landing
   bool have[N];
   bool exhausted = (SCHED == GRAY_SCHED_STATIC);
   unsigned long long c_steps = 0;
@@ -69,7 +72,7 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
 #pragma unroll
   for (int i = 0; i < 8; ++i) { y[i] = K.one; comp[i] = K.zero; }
 #pragma unroll
-  for (int l = 0; l < N; ++l) { have[l] = false; mirrored[l] = 0; idx[l] = 0; nst[l] = nst0[l] = iss[l] = 0; fstat[l] = GRAY_LIVE; }
+  for (int l = 0; l < N; ++l) { have[l] = false; landing[l] = 0; mirrored[l] = 0; idx[l] = 0; nst[l] = nst0[l] = iss[l] = 0; fstat[l] = GRAY_LIVE; }
 
   // HBM -> registers: photon want[l] into slot l (for the slots with want[l] < n), if it is live and has steps
   // left.  (t, r, theta, phi), k^mu -> the kernel's variables (gray_math.cuh): d = r - r_+ and theta folded into
@@ -99,6 +102,7 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
       idx[l] = p;
       nst[l] = nst0[l] = iss[l] = s;
       fstat[l] = GRAY_LIVE;
+      landing[l] = 0;
       have[l] = true;
     }
 #pragma unroll
@@ -160,7 +164,16 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
 #pragma unroll
       for (int l = 0; l < N; ++l) any |= have[l];
       if (any) {
-        const V dl = step_size<V, RULE>(K, y[1], y[5], y[6], y[7]);
+        V dl = step_size<V, RULE>(K, y[1], y[5], y[6], y[7]);
+        if (EQ && lnd) {
+          // landing on the equatorial plane: a Newton step dlambda = -(theta - pi/2) / k^theta instead of the rule
+          S dls[N], ths[N], khs[N];
+          vunpack(dl, dls); vunpack(y[2], ths); vunpack(y[6], khs);
+#pragma unroll
+          for (int l = 0; l < N; ++l)
+            if (landing[l]) dls[l] = -(ths[l] - S(1.57079632679489661923)) / khs[l];
+          vpack(dl, dls);
+        }
         if (!FROZEN) {
           bool rej[N];
           rk4_step<XI>(K, y, comp, dl, rej);
@@ -177,26 +190,52 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
           bool out_of_fold = false;
 #pragma unroll
           for (int l = 0; l < N; ++l) out_of_fold |= !(th[l] >= S(0) && th[l] <= S(1.57079632679489661923));
-          if (out_of_fold) {
+          const bool slow = out_of_fold || (EQ && lnd);
+          bool start[N];
+#pragma unroll
+          for (int l = 0; l < N; ++l) start[l] = false;
+          if (slow) {
             // eq. (3) remap and the fold, on the scalars of every slot (a slot without a photon carries junk,
-            // which is remapped too and never stored), then the packed values are rebuilt unconditionally
+            // which is remapped too and never stored), then the packed values are rebuilt unconditionally.
+            // stop_at_equator: a photon that crosses the plane is not folded but landed on it.
             S ph[N], kh[N], c2[N], c6[N];
             vunpack(y[3], ph); vunpack(y[6], kh); vunpack(comp[2], c2); vunpack(comp[6], c6);
 #pragma unroll
-            for (int l = 0; l < N; ++l) remap_theta(th[l], ph[l], kh[l], c2[l], c6[l], mirrored[l]);
+            for (int l = 0; l < N; ++l) {
+              const bool fold = !(EQ && have[l]);
+              const bool over = remap_theta(th[l], ph[l], kh[l], c2[l], c6[l], mirrored[l], fold);
+              start[l] = !fold && over && landing[l] == 0;
+            }
             vpack(y[2], th); vpack(y[3], ph); vpack(y[6], kh); vpack(comp[2], c2); vpack(comp[6], c6);
           }
           bool fin[N], any_fin = false;
 #pragma unroll
           for (int l = 0; l < N; ++l) {
             ++nst[l];
-            fin[l] = have[l] && (!(zz[l] == S(0) && rr[l] >= K.r_cap && rr[l] <= K.r_esc) || nst[l] == A.max_steps);
-            any_fin |= fin[l];
+            const bool bad_or_captured = !(zz[l] == S(0) && rr[l] >= K.r_cap);
+            bool f = have[l] && (bad_or_captured || !(rr[l] <= K.r_esc) || nst[l] == A.max_steps);
+            if (EQ && slow) {
+              if (landing[l] == 2) f = have[l];                              // second Newton step done: on the plane
+              else if (landing[l] == 1) { landing[l] = 2; f = false; }
+              else if (start[l] && !bad_or_captured) { landing[l] = 1; f = false; }
+            }
+            fin[l] = f;
+            any_fin |= f;
           }
           if (any_fin) {
 #pragma unroll
             for (int l = 0; l < N; ++l)
-              if (fin[l]) retire(l, state_status(zz[l], rr[l], K.r_cap, K.r_esc));
+              if (fin[l]) {
+                int st = state_status(zz[l], rr[l], K.r_cap, K.r_esc);
+                if (EQ && landing[l] == 2) st = zz[l] == S(0) ? GRAY_EQUATOR : GRAY_BAD;
+                landing[l] = 0;
+                retire(l, st);
+              }
+          }
+          if (EQ && (slow || any_fin)) {
+            lnd = false;
+#pragma unroll
+            for (int l = 0; l < N; ++l) lnd |= landing[l] != 0;
           }
         } else {
           V w[8], wc[8];
@@ -213,7 +252,7 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
 #pragma unroll
           for (int l = 0; l < N; ++l) {
             wm[l] = mirrored[l];
-            remap_theta(th[l], ph[l], kh[l], c2[l], c6[l], wm[l]);
+            remap_theta(th[l], ph[l], kh[l], c2[l], c6[l], wm[l], true);
             adv[l] = have[l] && fstat[l] == GRAY_LIVE;
           }
           vpack(w[2], th); vpack(w[3], ph); vpack(w[6], kh); vpack(wc[2], c2); vpack(wc[6], c6);
@@ -256,9 +295,9 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
   }
 }
 
-template <typename V, int RULE, int SCHED, bool FROZEN, bool XI>
+template <typename V, int RULE, int SCHED, bool FROZEN, bool XI, bool EQ>
 static int launch(const IntegrateArgs<V>& A, cudaStream_t stream) {
-  auto kern = integrate_kernel<V, RULE, SCHED, FROZEN, XI>;
+  auto kern = integrate_kernel<V, RULE, SCHED, FROZEN, XI, EQ>;
   constexpr unsigned long long per_block = (unsigned long long)kBlock * VT<V>::N;
   unsigned long long blocks_needed = (A.n + per_block - 1) / per_block;
   unsigned int grid;
@@ -279,8 +318,9 @@ static int launch(const IntegrateArgs<V>& A, cudaStream_t stream) {
 
 template <typename V, int RULE, int SCHED>
 static int dispatch_frozen(const IntegrateArgs<V>& A, bool frozen, cudaStream_t s) {
-  if (frozen) return launch<V, RULE, SCHED, true, false>(A, s);
-  return A.K.xi_eps > 0 ? launch<V, RULE, SCHED, false, true>(A, s) : launch<V, RULE, SCHED, false, false>(A, s);
+  if (frozen) return launch<V, RULE, SCHED, true, false, false>(A, s);
+  if (A.stop_eq) return A.K.xi_eps > 0 ? launch<V, RULE, SCHED, false, true, true>(A, s) : launch<V, RULE, SCHED, false, false, true>(A, s);
+  return A.K.xi_eps > 0 ? launch<V, RULE, SCHED, false, true, false>(A, s) : launch<V, RULE, SCHED, false, false, false>(A, s);
 }
 template <typename V, int RULE>
 static int dispatch_sched(const IntegrateArgs<V>& A, int sched, bool frozen, cudaStream_t s) {
@@ -300,6 +340,7 @@ static int integrate(const gray_state* st, uint64_t n, uint32_t max_steps, const
   A.n = n;
   A.max_steps = max_steps;
   A.refill_interval = p->refill_interval > 0 ? p->refill_interval : 8;
+  A.stop_eq = p->stop_at_equator != 0;
   const double a = st->a, rh = 1.0 + sqrt(1.0 - a * a);
   A.K = make_consts<V>(a, p->h, p->r_capture_factor > 0.0 ? p->r_capture_factor * rh : rh + p->horizon_delta,
                        p->r_escape_factor * st->r_obs, p->xi_epsilon);
@@ -325,6 +366,7 @@ int gray_integrate(gray_state* state, uint64_t n_photons, uint32_t max_steps, co
   if (params->refill_interval < 0) { set_error("refill_interval must be >= 0"); return GRAY_ERR_ARG; }
   if (!(params->xi_epsilon >= 0.0)) { set_error("xi_epsilon must be >= 0"); return GRAY_ERR_DOMAIN; }
   if (params->xi_epsilon > 0.0 && params->frozen) { set_error("xi_epsilon > 0 is not available together with frozen"); return GRAY_ERR_UNSUPPORTED; }
+  if (params->stop_at_equator && params->frozen) { set_error("stop_at_equator is not available together with frozen"); return GRAY_ERR_UNSUPPORTED; }
   if (params->photons_per_thread < 0 || params->photons_per_thread > 2) { set_error("photons_per_thread must be 0 (default), 1 or 2"); return GRAY_ERR_ARG; }
   if (params->photons_per_thread == 2 && state->prec != GRAY_F32) { set_error("photons_per_thread = 2 (packed FP32 instructions) needs GRAY_F32"); return GRAY_ERR_UNSUPPORTED; }
   if (!(params->h > 0.0) || !(params->r_escape_factor > 0.0) || params->r_capture_factor < 0.0 ||

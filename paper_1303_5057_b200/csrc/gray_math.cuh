@@ -303,9 +303,11 @@ GRAY_DEV double two_pi_minus(double x) { return (6.283185307179586232 - x) + 2.4
 // ---- theta remap, paper eq. (3), followed by the reflection that keeps th in [0, pi/2] ----------
 // One photon (scalar S).  Eq. (3) acts on the true polar angle.  For a mirrored photon (true angle
 // pi - th) the true angle exceeds pi when th < 0 and is negative when th > pi, so the sign of the phi
-// shift flips with it.
+// shift flips with it.  Returns whether the (eq. (3)-remapped) folded angle exceeds pi/2, i.e. whether the step
+// crossed the equatorial plane; the fold itself is applied only if `fold` (gray.h stop_at_equator lands the
+// photon on the plane instead).
 template <typename S>
-GRAY_DEV void remap_theta(S& th, S& ph, S& kh, S& c_th, S& c_kh, int& mirrored) {
+GRAY_DEV bool remap_theta(S& th, S& ph, S& kh, S& c_th, S& c_kh, int& mirrored, bool fold) {
   const S pi = S(3.14159265358979323846);
   const S shift = mirrored ? -pi : pi;
   if (th > pi) {
@@ -317,11 +319,13 @@ GRAY_DEV void remap_theta(S& th, S& ph, S& kh, S& c_th, S& c_kh, int& mirrored) 
     ph -= shift;
     kh = sneg(kh); c_th = sneg(c_th); c_kh = sneg(c_kh);
   }
-  if (th > S(1.57079632679489661923)) {
+  const bool over = th > S(1.57079632679489661923);      // the true polar angle has crossed the equatorial plane
+  if (over && fold) {
     th = pi_minus(th);
     kh = sneg(kh); c_th = sneg(c_th); c_kh = sneg(c_kh);
     mirrored ^= 1;
   }
+  return over;
 }
 
 // ---- non-finite detector: z = sum_i 0 * k^i is 0 iff the four momentum components are finite ------------

@@ -228,3 +228,40 @@ def test_pole_treatment_xi_monitor_matches_oracle_and_cures_the_pole_failures(pr
     assert cnt0["fallback_steps"] == 0 and cnt1["fallback_steps"] > 0
     assert np.sum(inside & (ref0 != o.CAPTURED)) > 0 and np.sum(inside & (st0 != g.CAPTURED)) > 0     # the failure
     assert np.sum(inside & (ref1 != o.CAPTURED)) == 0 and np.sum(inside & (st1 != g.CAPTURED)) == 0   # the cure
+
+
+@pytest.mark.parametrize("prec", [g.GRAY_F32, g.GRAY_F64])
+@pytest.mark.parametrize("a,inc", [(0.0, 60.0), (0.95, 60.0), (0.95, 0.0), (0.0, 0.0)])
+def test_equatorial_plane_projection_matches_oracle(prec, a, inc):
+    # NEXT-2: the paper's first benchmark (Fig. 3): a uniform image-plane grid projected onto the
+    # equatorial plane, a in {0, 0.95} x i in {0, 60 deg}.  Every ray ends CAPTURED or on the plane (EQUATOR).
+    nx, ny, W = 96, 61, 10.0
+    f32 = prec == g.GRAY_F32
+    b = g.PhotonBatch(nx * ny, prec)
+    g.gray_init_rays(b, a, wl.R_OBS, inc, W, nx, ny)
+    g.gray_integrate(b, max_steps=wl.MAX_STEPS, params=g.StepParams(rule=g.STEP_EQ2, stop_at_equator=True))
+    torch.cuda.synchronize()
+    y = torch.cat([b.x, b.k], dim=1).double().cpu().numpy()
+    st = b.status.cpu().numpy().astype(np.int32)
+    ns = b.steps.cpu().numpy().astype(np.int64)
+    ref = o.trace(a, wl.R_OBS, inc, W, nx, ny, rule=o.STEP_EQ2, init_f32=f32, threads=16, stop_at_equator=True)
+    assert set(np.unique(st)) <= {g.CAPTURED, g.EQUATOR} and (st == g.EQUATOR).mean() > 0.7
+    assert np.mean(st == ref["status"]) >= 0.999
+    same = (st == ref["status"]) & (ns == ref["steps"])
+    assert same.mean() > (0.99 if f32 else 0.999)
+    hit = same & (st == g.EQUATOR)
+    assert np.max(np.abs(y[hit, 2] - np.pi / 2)) < 2e-7                             # landed on the plane (two Newton steps)
+    dphi = np.abs(y[hit, 3] - ref["y"][hit, 3]) / np.maximum(1.0, np.abs(ref["y"][hit, 3]))
+    dr = np.abs(y[hit, 1] - ref["y"][hit, 1]) / ref["y"][hit, 1]
+    err = np.maximum(dr, dphi)
+    if f32:
+        assert np.quantile(err, 0.99) <= 2e-5 and err.max() <= 1e-3, (np.quantile(err, 0.99), err.max())
+    else:
+        assert np.quantile(err, 0.99) <= 1e-10 and err.max() <= 1e-8, (np.quantile(err, 0.99), err.max())
+    # schedules and packing do not change a bit here either
+    b2 = g.PhotonBatch(nx * ny, prec)
+    g.gray_init_rays(b2, a, wl.R_OBS, inc, W, nx, ny)
+    g.gray_integrate(b2, max_steps=wl.MAX_STEPS, params=g.StepParams(rule=g.STEP_EQ2, stop_at_equator=True, schedule=g.SCHED_STATIC,
+                                                                     photons_per_thread=1))
+    assert torch.equal(b.x.view(torch.uint8), b2.x.view(torch.uint8)) and torch.equal(b.status, b2.status)
+    assert torch.equal(b.steps, b2.steps)

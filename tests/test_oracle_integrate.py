@@ -242,3 +242,67 @@ def test_pole_treatment_xi_monitor_cures_the_pole_failures():
     c2 = o.trace(a, 1000.0, inc, W, nx, nx, idx=idx2, rule=o.STEP_EQ2, xi_eps=1e-3)
     esc = p2["status"] == o.ESCAPED
     assert esc.any() and np.array_equal(p2["y"][esc], c2["y"][esc]) and np.array_equal(p2["steps"][esc], c2["steps"][esc])
+
+
+def test_equatorial_projection_schwarzschild_node_line_and_orbit_integral():
+    # NEXT-2: follow rays to the equatorial plane.  Pins for a = 0, where the motion is planar:
+    # (i) the plane of the orbit contains the origin, the observer direction o and the pixel offset, so its line of
+    # nodes with the equatorial plane - hence phi at the crossing - is pure geometry; (ii) the crossing radius
+    # follows from the textbook orbit integral  psi = int du / sqrt(1/b^2 - u^2 (1 - 2u))  over the in-plane
+    # angle psi between the starting point and the node.
+    from scipy import integrate as sint, optimize
+    a, inc_deg, r_obs = 0.0, 60.0, 1000.0
+    inc = np.radians(inc_deg)
+    o_hat = np.array([np.sin(inc), 0.0, np.cos(inc)])
+    b_hat = np.array([-np.cos(inc), 0.0, np.sin(inc)])
+    y_hat = np.array([0.0, 1.0, 0.0])
+    checked = 0
+    for al, be in [(6.0, 9.0), (-8.0, 7.0), (3.0, 9.5), (-9.0, 4.0), (9.5, 9.5)]:
+        y0 = o.init_ray(a, r_obs, inc_deg, al, be)
+        y, st, n = o.integrate(a, y0, 1 / 32, 1.01 * 2.0, 1.01 * r_obs, o.STEP_EQ2, 20000, stop_at_equator=True)
+        assert st == o.EQUATOR and abs(y[2] - np.pi / 2) < 1e-8
+        X0 = r_obs * o_hat + al * y_hat + be * b_hat
+        nrm = np.cross(o_hat, al * y_hat + be * b_hat)
+        node = np.cross([0.0, 0.0, 1.0], nrm)
+        node /= np.linalg.norm(node)
+        hit = np.array([np.cos(y[3]), np.sin(y[3]), 0.0])
+        s = np.sign(hit @ node)
+        assert abs(np.cross(hit, node)[2]) < 2e-6                           # (i) phi on the line of nodes
+        psi = np.arccos(np.clip((X0 / np.linalg.norm(X0)) @ (s * node), -1, 1))
+        E, L, Q, _ = o.invariants(a, y0)
+        b = np.sqrt(Q + L * L) / E                                            # total angular momentum / energy
+        f = lambda u: 1.0 / (b * b) - u * u * (1.0 - 2.0 * u)
+        u0 = 1.0 / y0[1]
+        um = optimize.brentq(f, 0.5 / b, 1.0 / 3.0, xtol=1e-16)
+        def leg(uc):      # in-plane angle between u = uc and the periapsis u = um; u = um - s^2 removes the end-point singularity
+            g = lambda t: 2.0 * t / np.sqrt(max(f(um - t * t), 1e-300))
+            return sint.quad(g, 0.0, np.sqrt(um - uc), epsabs=1e-13, epsrel=1e-13, limit=400)[0]
+
+        if psi <= leg(u0):                                                    # node reached on the way in
+            uc = optimize.brentq(lambda u: leg(u0) - leg(u) - psi, u0, um, xtol=1e-15)
+        else:                                                                 # ... or on the way out
+            uc = optimize.brentq(lambda u: leg(u) - (psi - leg(u0)), 1e-9, um, xtol=1e-15)
+        assert abs(y[1] - 1.0 / uc) < 2e-6 / uc, (al, be, y[1], 1.0 / uc)     # (ii) crossing radius
+        checked += 1
+    assert checked == 5
+
+
+def test_equatorial_projection_kerr_invariants_and_symmetry():
+    # Kerr: the reported crossing state conserves E, L_z and Q to the scheme's truncation error, the
+    # map is symmetric under (i, beta) -> (180 - i, -beta), and rays aimed inside the shadow are still CAPTURED
+    # unless they reach the plane first.  Beyond this the Kerr crossing radius is parity-unpinned.
+    a = 0.95
+    for al, be in [(5.0, 8.0), (-7.0, 6.0), (9.0, -9.0)]:
+        y0 = o.init_ray(a, 1000.0, 60.0, al, be)
+        y, st, n = o.integrate(a, y0, 1 / 32, 1.01 * o.horizon(a), 1010.0, o.STEP_EQ2, 20000, stop_at_equator=True)
+        assert st == o.EQUATOR
+        i0, i1 = o.invariants(a, y0), o.invariants(a, y)
+        assert abs(y[2] - np.pi / 2) < 1e-8
+        assert np.all(np.abs(np.array(i1[:3]) - np.array(i0[:3])) < 2e-5 * np.maximum(1.0, np.abs(i0[:3])))
+        y2, st2, n2 = o.integrate(a, o.init_ray(a, 1000.0, 120.0, al, -be), 1 / 32, 1.01 * o.horizon(a), 1010.0, o.STEP_EQ2,
+                                  20000, stop_at_equator=True)
+        assert st2 == o.EQUATOR and n2 == n and np.allclose(y[[1, 3]], y2[[1, 3]], rtol=1e-9, atol=1e-9)
+    r = o.trace(a, 1000.0, 60.0, 10.0, 32, 32, rule=o.STEP_EQ2, stop_at_equator=True, threads=8)
+    assert set(np.unique(r["status"])) == {o.CAPTURED, o.EQUATOR}
+    plain = o.trace(a, 1000.0, 60.0, 10.0, 32, 32, rule=o.STEP_EQ2, threads=8)
+    assert np.all(plain["status"][r["status"] == o.CAPTURED] == o.CAPTURED)   # captured without touching the plane
