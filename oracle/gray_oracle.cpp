@@ -66,6 +66,11 @@ void gray_oracle_pixel_grid(double W, int64_t nx, int64_t ny, uint64_t p, double
   go::pixel_grid(W, nx, ny, p, alpha, beta);
 }
 
+void gray_oracle_pixel_polar(double R_lo, double R_hi, int64_t n_R, int64_t n_theta, uint64_t p, double* alpha,
+                             double* beta) {
+  go::pixel_polar(R_lo, R_hi, n_R, n_theta, p, alpha, beta);
+}
+
 void gray_oracle_pixel_random(uint64_t seed, uint64_t p, double W, double* alpha, double* beta) {
   go::pixel_random(seed, p, W, alpha, beta);
 }
@@ -94,6 +99,7 @@ int gray_oracle_integrate(double a, double* y, double h, double r_capture, doubl
 // indices are idx[0..n_idx) (idx == NULL: photons 0..n_idx-1).
 //   nx > 0  : grid workload, nx x ny pixel centres over [-W, W]^2
 //   nx == 0 : random workload keyed by (seed, photon index)
+//   nx < 0  : polar grid of -nx radii in (polar_R_lo, W) x ny angles in [0, pi] (gray_oracle::pixel_polar)
 //   capture radius = cap_factor * r_h if cap_factor > 0, else r_h + horizon_delta
 //   init_f32 != 0 : the initial state is rounded to fp32 before integrating (what
 //                   the fp32 build stores; the integration itself stays double)
@@ -107,7 +113,8 @@ int gray_oracle_trace(double a, double r_obs, double inc_deg, double W, int64_t 
                       uint64_t seed, const uint64_t* idx, uint64_t n_idx, double h, double cap_factor,
                       double esc_factor, double horizon_delta, int rule, uint32_t max_steps,
                       int init_f32, const int64_t* force_steps, int n_threads, double* y0_out,
-                      double* y_out, int32_t* status_out, uint32_t* steps_out, double xi_eps, int stop_at_equator) {
+                      double* y_out, int32_t* status_out, uint32_t* steps_out, double xi_eps, int stop_at_equator,
+                      double polar_R_lo) {
   if (n_threads < 1) n_threads = 1;
   double rh = go::horizon(a);
   go::StepParams sp{h, cap_factor > 0 ? cap_factor * rh : rh + horizon_delta, esc_factor * r_obs, rule, xi_eps,
@@ -117,7 +124,8 @@ int gray_oracle_trace(double a, double r_obs, double inc_deg, double W, int64_t 
     for (uint64_t j = lo; j < hi; ++j) {
       uint64_t p = idx ? idx[j] : j;
       double al, be, y[8];
-      if (nx > 0) go::pixel_grid(W, nx, ny, p, &al, &be);
+      if (nx < 0) go::pixel_polar(polar_R_lo, W, -nx, ny, p, &al, &be);
+      else if (nx > 0) go::pixel_grid(W, nx, ny, p, &al, &be);
       else go::pixel_random(seed, p, W, &al, &be);
       go::init_ray(a, r_obs, inc, al, be, y);
       if (init_f32)
@@ -208,6 +216,43 @@ void gray_oracle_shadow_stats(const uint8_t* captured, int64_t nx, int64_t ny, d
   var = n_angles > 0 ? var / n_angles : 0.0;
   out[6] = mean;
   out[7] = 2.0 * std::sqrt(var);
+}
+
+// Photon-ring statistics on the paper's polar grid (eqs. 6-10; NEXT-4).  captured[k*n_R+j] != 0 marks a
+// captured ray at angle vartheta_k = k pi / (n_theta - 1), radius cell j of (R_lo, R_hi).
+//   radius[k] = ring radius on spoke k: the outer edge of the last captured cell counted from the inside while the
+//               cells are captured (R_lo if the innermost cell is not captured)
+//   out[0], out[1] = alpha_min = -radius[n_theta-1], alpha_max = radius[0]  (the ring meets the alpha axis there)
+//   out[2] D (eq. 6); with R = [(alpha_0 - c)^2 + beta_0^2]^(1/2) about the ring centre c = (alpha_min + alpha_max)/2
+//   out[3] <R> (eq. 7), out[4] A (eq. 8): the integrals over [0, 2 pi] are twice those over [0, pi] (the image is
+//   symmetric under beta -> -beta), evaluated by the trapezoidal rule on the n_theta angles.
+void gray_oracle_ring_polar(const uint8_t* captured, int64_t n_R, int64_t n_theta, double R_lo, double R_hi,
+                            double* radius, double* out) {
+  double dR = (R_hi - R_lo) / (double)n_R;
+  std::vector<double> rad(n_theta), R(n_theta);
+  for (int64_t k = 0; k < n_theta; ++k) {
+    int64_t j = 0;
+    while (j < n_R && captured[k * n_R + j]) ++j;
+    rad[k] = R_lo + (double)j * dR;
+    if (radius) radius[k] = rad[k];
+  }
+  double amax = rad[0], amin = -rad[n_theta - 1];
+  double c = (amin + amax) / 2.0;
+  for (int64_t k = 0; k < n_theta; ++k) {
+    double vt = (double)k * (kPi / (double)(n_theta - 1));
+    double x = rad[k] * std::cos(vt) - c, y = rad[k] * std::sin(vt);
+    R[k] = std::sqrt(x * x + y * y);
+  }
+  auto trapz_mean = [&](const std::vector<double>& f) {
+    double sum = 0;
+    for (int64_t k = 0; k < n_theta; ++k) sum += (k == 0 || k == n_theta - 1 ? 0.5 : 1.0) * f[k];
+    return sum / (double)(n_theta - 1);
+  };
+  double mean = trapz_mean(R);
+  std::vector<double> dev(n_theta);
+  for (int64_t k = 0; k < n_theta; ++k) dev[k] = (R[k] - mean) * (R[k] - mean);
+  out[0] = amin; out[1] = amax; out[2] = std::fabs(amin + amax) / 2.0; out[3] = mean;
+  out[4] = 2.0 * std::sqrt(trapz_mean(dev));
 }
 
 // Operation tally of one photon-step (step size + RK4 step + remap) at state y.

@@ -185,6 +185,18 @@ inline void pixel_grid(double W, int64_t nx, int64_t ny, uint64_t p, double* alp
   *beta = -W + ((double)row + 0.5) * (2.0 * W / (double)ny);
 }
 
+// Polar image-plane grid of the paper's photon-ring study ("a grid of 6000 x 181 rays in the polar
+// domain (1.5, 7.5) x [0, pi]"; NEXT-4).  Reading (R20): the open radial interval is sampled at the n_R
+// cell centres, the closed angular interval at n_theta equally spaced angles including both ends; photon index
+// p = k n_R + j (angle slow); alpha = R cos(vartheta), beta = R sin(vartheta) (eqs. 9-10).
+inline void pixel_polar(double R_lo, double R_hi, int64_t n_R, int64_t n_theta, uint64_t p, double* alpha, double* beta) {
+  uint64_t j = p % (uint64_t)n_R, k = p / (uint64_t)n_R;
+  double R = R_lo + ((double)j + 0.5) * ((R_hi - R_lo) / (double)n_R);
+  double vt = (double)k * (3.14159265358979323846 / (double)(n_theta - 1));
+  *alpha = R * cos(vt);
+  *beta = R * sin(vt);
+}
+
 // Stateless counter-based pixel generator for the throughput workload (C4):
 // a 64-bit mix of (seed, p); two 24-bit integers u, v from it; the pixel is the
 // fp32 rounding of (2u + 1 - 2^24) W 2^-24.  (DESIGN.md input recipe.)

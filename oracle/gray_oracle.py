@@ -29,6 +29,7 @@ def lib():
         L.gray_oracle_invariants.argtypes = [C.c_double, _dp, _dp]
         L.gray_oracle_pixel_grid.argtypes = [C.c_double, C.c_int64, C.c_int64, C.c_uint64, _dp, _dp]
         L.gray_oracle_pixel_random.argtypes = [C.c_uint64, C.c_uint64, C.c_double, _dp, _dp]
+        L.gray_oracle_pixel_polar.argtypes = [C.c_double, C.c_double, C.c_int64, C.c_int64, C.c_uint64, _dp, _dp]
         L.gray_oracle_init_ray.argtypes = [C.c_double] * 5 + [_dp]
         L.gray_oracle_step_size.restype = C.c_double
         L.gray_oracle_step_size.argtypes = [C.c_double, _dp, C.c_double, C.c_int]
@@ -42,10 +43,12 @@ def lib():
                                                             C.c_uint64, C.c_double, C.c_double, C.c_double,
                                                             C.c_double, C.c_int, C.c_uint32, C.c_int,
                                                             C.c_void_p, C.c_int, C.c_void_p, C.c_void_p,
-                                                            C.c_void_p, C.c_void_p, C.c_double, C.c_int]
+                                                            C.c_void_p, C.c_void_p, C.c_double, C.c_int, C.c_double]
         L.gray_oracle_hardware_threads.restype = C.c_int
         L.gray_oracle_shadow_stats.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_double, C.c_int32,
                                                C.c_void_p, C.c_void_p]
+        L.gray_oracle_ring_polar.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_double, C.c_double, C.c_void_p,
+                                             C.c_void_p]
         L.gray_oracle_op_tally.argtypes = [C.c_double, _dp, C.c_double, C.c_int, C.POINTER(C.c_uint64)]
         _lib = L
     return _lib
@@ -138,16 +141,21 @@ def hardware_threads():
 
 def trace(a, r_obs, inc_deg, W, nx=0, ny=0, seed=0, idx=None, n=None, h=1.0 / 32, cap_factor=1.01,
           esc_factor=1.01, horizon_delta=1e-6, rule=STEP_EQ2, max_steps=20000, init_f32=False,
-          force_steps=None, threads=1, want_y0=True, xi_eps=0.0, stop_at_equator=False):
+          force_steps=None, threads=1, want_y0=True, xi_eps=0.0, stop_at_equator=False, polar=None):
     """Initialise and integrate a batch of photons; see gray_oracle_trace in gray_oracle.cpp.
+    polar = (R_lo, R_hi, n_R, n_theta) selects the paper's polar image-plane grid (W, nx, ny are then ignored).
 
     Returns dict(y0, y, status, steps).
     """
+    R_lo = 0.0
+    if polar is not None:
+        R_lo, W, n_R, ny = polar
+        nx = -int(n_R)
     if idx is not None:
         idx = np.ascontiguousarray(idx, dtype=np.uint64)
         n = idx.size
     elif n is None:
-        n = nx * ny
+        n = abs(nx) * ny
     y0 = np.zeros((n, 8)) if want_y0 else None
     y = np.zeros((n, 8))
     status = np.zeros(n, dtype=np.int32)
@@ -160,7 +168,7 @@ def trace(a, r_obs, inc_deg, W, nx=0, ny=0, seed=0, idx=None, n=None, h=1.0 / 32
                             horizon_delta, rule, max_steps, int(bool(init_f32)),
                             force_steps.ctypes.data if force_steps is not None else None, threads,
                             y0.ctypes.data if y0 is not None else None, y.ctypes.data,
-                            status.ctypes.data, steps.ctypes.data, xi_eps, int(bool(stop_at_equator)))
+                            status.ctypes.data, steps.ctypes.data, xi_eps, int(bool(stop_at_equator)), R_lo)
     return dict(y0=y0, y=y, status=status, steps=steps)
 
 
@@ -175,6 +183,22 @@ def shadow_stats(captured, W, n_angles):
     keys = ["area", "centroid_alpha", "centroid_beta", "alpha_min", "alpha_max", "D", "R_mean", "A",
             "n_captured"]
     return dict(zip(keys, out.tolist())), radius
+
+
+def ring_polar(captured, R_lo, R_hi):
+    """captured: (n_theta, n_R) uint8.  Returns (dict(alpha_min, alpha_max, D, R_mean, A), radius[n_theta])."""
+    captured = np.ascontiguousarray(captured, dtype=np.uint8)
+    n_theta, n_R = captured.shape
+    radius = np.zeros(n_theta)
+    out = np.zeros(5)
+    lib().gray_oracle_ring_polar(captured.ctypes.data, n_R, n_theta, R_lo, R_hi, radius.ctypes.data, out.ctypes.data)
+    return dict(zip(["alpha_min", "alpha_max", "D", "R_mean", "A"], out.tolist())), radius
+
+
+def pixel_polar(R_lo, R_hi, n_R, n_theta, p):
+    al, be = C.c_double(), C.c_double()
+    lib().gray_oracle_pixel_polar(R_lo, R_hi, n_R, n_theta, p, C.byref(al), C.byref(be))
+    return al.value, be.value
 
 
 def op_tally(a, y, h, rule):

@@ -123,3 +123,27 @@ def schwarzschild_dphi(b, r_start, r_end):
         return val
 
     return leg(1.0 / r_start) + leg(1.0 / r_end)
+
+
+def bardeen_ring_polar(a, inc_deg, n_theta=181):
+    """The paper's ring statistics (eqs. 6-10) of the closed-form critical curve, sampled like the paper's
+    polar grid: spokes vartheta_k = k pi / (n_theta - 1) about the image origin, R about the ring centre
+    ((alpha_min + alpha_max)/2, 0), integrals over [0, pi] by the trapezoidal rule.  i = 0 and a = 0 are the circles
+    sqrt(eta(xi = 0) + a^2) and sqrt(27)."""
+    vt = np.pi * np.arange(n_theta) / (n_theta - 1)
+    if a == 0.0:
+        rho = np.full(n_theta, np.sqrt(27.0))
+    elif inc_deg == 0.0:
+        lo, hi = photon_orbit_radii(a)
+        rp = optimize.brentq(lambda r: xi_eta(a, r)[0], lo, hi, xtol=1e-15)
+        rho = np.full(n_theta, np.sqrt(xi_eta(a, rp)[1] + a * a))
+    else:
+        rho = bardeen_rho(a, inc_deg, vt)
+    amax, amin = rho[0], -rho[-1]
+    c = 0.5 * (amin + amax)
+    R = np.hypot(rho * np.cos(vt) - c, rho * np.sin(vt))
+    w = np.ones(n_theta)
+    w[0] = w[-1] = 0.5
+    mean = np.sum(w * R) / (n_theta - 1)
+    A = 2.0 * np.sqrt(np.sum(w * (R - mean) ** 2) / (n_theta - 1))
+    return dict(alpha_min=amin, alpha_max=amax, D=abs(c), R_mean=mean, A=A), rho

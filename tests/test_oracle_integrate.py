@@ -306,3 +306,43 @@ def test_equatorial_projection_kerr_invariants_and_symmetry():
     assert set(np.unique(r["status"])) == {o.CAPTURED, o.EQUATOR}
     plain = o.trace(a, 1000.0, 60.0, 10.0, 32, 32, rule=o.STEP_EQ2, threads=8)
     assert np.all(plain["status"][r["status"] == o.CAPTURED] == o.CAPTURED)   # captured without touching the plane
+
+
+def test_polar_grid_and_ring_statistics_on_a_synthetic_disc():
+    # NEXT-4: polar grid geometry, and eqs. (6)-(10) on an exact shape: a disc of radius 3 centred at (1, 0)
+    # has alpha_min = -2, alpha_max = 4, D = 1, R = 3 on every spoke, A = 0.
+    R_lo, R_hi, n_R, n_th = 1.5, 7.5, 6000, 181
+    al, be = o.pixel_polar(R_lo, R_hi, n_R, n_th, 0)
+    assert abs(al - 1.5005) < 1e-12 and be == 0.0
+    al, be = o.pixel_polar(R_lo, R_hi, n_R, n_th, 90 * n_R + 2999)
+    assert abs(al) < 1e-12 and abs(be - (1.5 + 2999.5e-3)) < 1e-12           # vartheta = pi/2, mid radius
+    al, be = o.pixel_polar(R_lo, R_hi, n_R, n_th, 180 * n_R + 5999)
+    assert abs(al + 7.4995) < 1e-12 and abs(be) < 1e-12                         # vartheta = pi, outermost cell
+    vt = np.pi * np.arange(n_th) / (n_th - 1)
+    Rc = R_lo + (np.arange(n_R) + 0.5) * (R_hi - R_lo) / n_R
+    A_, B_ = Rc[None, :] * np.cos(vt)[:, None], Rc[None, :] * np.sin(vt)[:, None]
+    disc = (np.hypot(A_ - 1.0, B_) < 3.0).astype(np.uint8)
+    st, radius = o.ring_polar(disc, R_lo, R_hi)
+    exact = np.cos(vt) + np.sqrt(9.0 - np.sin(vt) ** 2)
+    assert np.max(np.abs(radius - exact)) <= 1.0e-3 + 1e-12                     # one radial cell
+    assert abs(st["alpha_min"] + 2) < 1e-3 and abs(st["alpha_max"] - 4) < 1e-3 and abs(st["D"] - 1) < 1e-3
+    assert abs(st["R_mean"] - 3) < 1e-3 and st["A"] < 1.5e-3
+
+
+@pytest.mark.parametrize("a,inc", [(0.9, 60.0), (1 - 10 ** (-10 / 5), 90.0), (0.6019, 0.0)])
+def test_polar_ring_study_against_bardeen_and_paper_fits(a, inc):
+    # the paper's photon-ring study on a coarser polar grid (600 x 37), with the xi monitor as in the
+    # paper; i = 0 needs it: every ray of a face-on image has L_z = 0 and passes over the pole
+    R_lo, R_hi, n_R, n_th = 1.5, 7.5, 600, 37
+    res = o.trace(a, 1000.0, inc, 0, polar=(R_lo, R_hi, n_R, n_th), rule=o.STEP_EQ2, xi_eps=1e-3, threads=8, want_y0=False)
+    assert not np.any(res["status"] == o.BAD) and not np.any(res["status"] == o.LIVE)
+    cap = (res["status"] == o.CAPTURED).reshape(n_th, n_R).astype(np.uint8)
+    st, radius = o.ring_polar(cap, R_lo, R_hi)
+    ex, rho = cf.bardeen_ring_polar(a, inc, n_th)
+    dR = (R_hi - R_lo) / n_R
+    assert np.max(np.abs(radius - rho)) < 1.0 * dR
+    for k in ("alpha_min", "alpha_max", "D", "R_mean"):
+        assert abs(st[k] - ex[k]) < dR, k
+    assert abs(st["A"] - ex["A"]) < dR
+    Rf, Af = _paper_fit(a, inc)                                                # eqs. (11)-(14): soft, they are fits
+    assert abs(st["R_mean"] - Rf) < 0.04 and abs(st["A"] - Af) < 0.04
