@@ -71,7 +71,7 @@ typedef enum { GRAY_LIVE = 0, GRAY_CAPTURED = 1, GRAY_ESCAPED = 2, GRAY_BAD = 3,
  * Per-photon results are bit-identical for both and for any refill_interval.                       */
 typedef enum { GRAY_SCHED_REFILL = 0, GRAY_SCHED_STATIC = 1 } gray_schedule;
 
-typedef enum { GRAY_PIXELS_GRID = 0, GRAY_PIXELS_RANDOM = 1 } gray_pixels;
+typedef enum { GRAY_PIXELS_GRID = 0, GRAY_PIXELS_RANDOM = 1, GRAY_PIXELS_POLAR = 2 } gray_pixels;
 
 /* A batch of photons.  The caller fills the four pointers, n and prec; gray_init_rays* fills the
  * rest (the description of the image plane), which gray_integrate / gray_classify /
@@ -91,6 +91,7 @@ typedef struct {
   int32_t nx, ny;         /* grid workload: pixels per row (alpha, fast) and rows (beta, slow)       */
   uint64_t seed;          /* random workload: key of the counter-based pixel generator               */
   uint64_t p0;            /* global index of photon 0 of this batch (sharding across GPUs / chunks)  */
+  double r_lo;            /* polar workload: inner radius of the image-plane annulus (outer = half_width) */
 } gray_state;
 
 /* Image plane -> initial photon states ("initial conditions ... as in Psaltis & Johannsen
@@ -108,6 +109,15 @@ GRAY_API int gray_init_rays(gray_state* state, double a, double r_obs, double in
                    int32_t nx, int32_t ny, uint64_t p0, void* cuda_stream);
 GRAY_API int gray_init_rays_random(gray_state* state, double a, double r_obs, double inc_deg, double half_width,
                           uint64_t seed, uint64_t p0, void* cuda_stream);
+
+/* The paper's polar image-plane grid (photon-ring study: "6000 x 181 rays in the polar domain
+ * (1.5, 7.5) x [0, pi]"; reading R20).  Photon p of the image: j = p mod n_R, k = p / n_R,
+ *   R_j = R_lo + (j + 1/2) (R_hi - R_lo) / n_R,  vartheta_k = k pi / (n_theta - 1),
+ *   alpha = R cos(vartheta), beta = R sin(vartheta)  (eqs. 9-10).
+ * Everything else as gray_init_rays (state->nx = n_R, ny = n_theta, half_width = R_hi, r_lo = R_lo).
+ * Requires n_theta >= 2, 0 <= R_lo < R_hi, p0 + n <= n_R * n_theta.                                  */
+GRAY_API int gray_init_rays_polar(gray_state* state, double a, double r_obs, double inc_deg, double R_lo, double R_hi,
+                         int32_t n_R, int32_t n_theta, uint64_t p0, void* cuda_stream);
 
 typedef struct {
   double h;                  /* step parameter, the paper's Delta ~ 1/32                      */
@@ -191,6 +201,19 @@ typedef struct {
 GRAY_API int gray_shadow_edge(const gray_state* state, int32_t n_angles, double* radius_dev,
                      gray_shadow_stats* stats_host, void* workspace_dev, size_t workspace_bytes,
                      void* cuda_stream);
+
+/* Photon-ring statistics of a polar image (eqs. 6-10).  radius[k] = ring radius on spoke k: the outer
+ * edge of the outermost captured cell (R_lo if none is captured).  alpha_max = radius[0], alpha_min = -radius[n_theta - 1]; D = |alpha_min + alpha_max| / 2
+ * (eq. 6); R = [(alpha_0 - c)^2 + beta_0^2]^(1/2) about the ring centre c = (alpha_min + alpha_max)/2; R_mean (eq. 7)
+ * and A (eq. 8) with the integrals over [0, pi] (the image is symmetric under beta -> -beta) by the trapezoidal
+ * rule on the n_theta spokes.  bridge_axis != 0 (n_theta odd): the middle spoke vartheta = pi/2 has alpha = 0, its rays
+ * run through the spin axis, the degenerate case of Boyer-Lindquist coordinates in which the second-order equations
+ * lose rays even with the xi monitor (R20); its radius is then replaced by the mean of its two neighbours
+ * before the statistics are formed.  Requires a full polar batch.  radius_dev (n_theta doubles) may be NULL.
+ * Synchronises the stream.                                                                             */
+typedef struct { double alpha_min, alpha_max, D, R_mean, A; } gray_ring_stats;
+GRAY_API int gray_ring_polar(const gray_state* state, int32_t bridge_axis, double* radius_dev, gray_ring_stats* stats_host,
+                    void* workspace_dev, size_t workspace_bytes, void* cuda_stream);
 
 /* End-to-end variant with HOST buffers (bench.py's `e2e` figure).  n photons whose initial states are
  * x_in_host / k_in_host (n x 4 scalars of `prec`, status LIVE, steps 0 implied) are streamed through

@@ -220,22 +220,31 @@ void gray_oracle_shadow_stats(const uint8_t* captured, int64_t nx, int64_t ny, d
 
 // Photon-ring statistics on the paper's polar grid (eqs. 6-10; NEXT-4).  captured[k*n_R+j] != 0 marks a
 // captured ray at angle vartheta_k = k pi / (n_theta - 1), radius cell j of (R_lo, R_hi).
-//   radius[k] = ring radius on spoke k: the outer edge of the last captured cell counted from the inside while the
-//               cells are captured (R_lo if the innermost cell is not captured)
+//   radius[k] = ring radius on spoke k: the outer edge of the outermost captured cell (R_lo if none is captured).
+//               Scanning from the outside keeps the outline insensitive to a stray non-captured ray inside the
+//               shadow (the axis spoke vartheta = pi/2 of the paper's grid has alpha = 0: its rays run through the
+//               pole exactly, the degenerate case of Boyer-Lindquist coordinates, R20)
 //   out[0], out[1] = alpha_min = -radius[n_theta-1], alpha_max = radius[0]  (the ring meets the alpha axis there)
 //   out[2] D (eq. 6); with R = [(alpha_0 - c)^2 + beta_0^2]^(1/2) about the ring centre c = (alpha_min + alpha_max)/2
 //   out[3] <R> (eq. 7), out[4] A (eq. 8): the integrals over [0, 2 pi] are twice those over [0, pi] (the image is
 //   symmetric under beta -> -beta), evaluated by the trapezoidal rule on the n_theta angles.
+//   bridge_axis != 0 (n_theta odd): the radius of the middle spoke vartheta = pi/2 is replaced by the mean of its two
+//               neighbours before anything else is computed (and returned so in radius[]).
 void gray_oracle_ring_polar(const uint8_t* captured, int64_t n_R, int64_t n_theta, double R_lo, double R_hi,
-                            double* radius, double* out) {
+                            int bridge_axis, double* radius, double* out) {
   double dR = (R_hi - R_lo) / (double)n_R;
   std::vector<double> rad(n_theta), R(n_theta);
   for (int64_t k = 0; k < n_theta; ++k) {
-    int64_t j = 0;
-    while (j < n_R && captured[k * n_R + j]) ++j;
+    int64_t j = n_R;
+    while (j > 0 && !captured[k * n_R + j - 1]) --j;
     rad[k] = R_lo + (double)j * dR;
-    if (radius) radius[k] = rad[k];
   }
+  if (bridge_axis && n_theta >= 3 && (n_theta % 2) == 1) {
+    int64_t m = (n_theta - 1) / 2;
+    rad[m] = 0.5 * (rad[m - 1] + rad[m + 1]);
+  }
+  if (radius)
+    for (int64_t k = 0; k < n_theta; ++k) radius[k] = rad[k];
   double amax = rad[0], amin = -rad[n_theta - 1];
   double c = (amin + amax) / 2.0;
   for (int64_t k = 0; k < n_theta; ++k) {

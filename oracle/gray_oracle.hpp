@@ -29,6 +29,8 @@
 //   equatorial projection : a = 0 line of nodes and orbit integral (phi, r at the
 //                           crossing to 2e-6); Kerr: invariants at the landed state,
 //                           reflection symmetry
+//   polar grid, ring stats: exact disc; Bardeen curve sampled on the same spokes;
+//                           the paper's fits eqs. 11-14 (soft)
 //   shadow statistics     : Bardeen closed-form curve (area, alpha extent, D,
 //                           <R>, A), an exact synthetic disc, paper eqs. 11-14
 // Parity unpinned (GPU-vs-oracle only): the final state of CAPTURED rays at

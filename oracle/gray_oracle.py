@@ -47,8 +47,8 @@ def lib():
         L.gray_oracle_hardware_threads.restype = C.c_int
         L.gray_oracle_shadow_stats.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_double, C.c_int32,
                                                C.c_void_p, C.c_void_p]
-        L.gray_oracle_ring_polar.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_double, C.c_double, C.c_void_p,
-                                             C.c_void_p]
+        L.gray_oracle_ring_polar.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_double, C.c_double, C.c_int,
+                                             C.c_void_p, C.c_void_p]
         L.gray_oracle_op_tally.argtypes = [C.c_double, _dp, C.c_double, C.c_int, C.POINTER(C.c_uint64)]
         _lib = L
     return _lib
@@ -185,13 +185,14 @@ def shadow_stats(captured, W, n_angles):
     return dict(zip(keys, out.tolist())), radius
 
 
-def ring_polar(captured, R_lo, R_hi):
+def ring_polar(captured, R_lo, R_hi, bridge_axis=False):
     """captured: (n_theta, n_R) uint8.  Returns (dict(alpha_min, alpha_max, D, R_mean, A), radius[n_theta])."""
     captured = np.ascontiguousarray(captured, dtype=np.uint8)
     n_theta, n_R = captured.shape
     radius = np.zeros(n_theta)
     out = np.zeros(5)
-    lib().gray_oracle_ring_polar(captured.ctypes.data, n_R, n_theta, R_lo, R_hi, radius.ctypes.data, out.ctypes.data)
+    lib().gray_oracle_ring_polar(captured.ctypes.data, n_R, n_theta, R_lo, R_hi, int(bool(bridge_axis)), radius.ctypes.data,
+                                 out.ctypes.data)
     return dict(zip(["alpha_min", "alpha_max", "D", "R_mean", "A"], out.tolist())), radius
 
 

@@ -12,7 +12,7 @@ struct InitArgs {
   uint8_t* status;
   uint32_t* steps;
   unsigned long long n, p0, seed;
-  double a, r_obs, sin_i, cos_i, W;
+  double a, r_obs, sin_i, cos_i, W, R_lo;
   unsigned long long nx, ny;
 };
 
@@ -31,7 +31,17 @@ __global__ void __launch_bounds__(256) init_kernel(const __grid_constant__ InitA
   if (j >= A.n) return;
   const unsigned long long p = A.p0 + j;
   double alpha, beta;
-  if (PIXELS == GRAY_PIXELS_GRID) {
+  if (PIXELS == GRAY_PIXELS_POLAR) {
+    // nx radii (cell centres of (R_lo, W)), ny angles in [0, pi] including both ends; explicit roundings
+    const unsigned long long jr = p % A.nx, kt = p / A.nx;
+    const double dR = __ddiv_rn(__dadd_rn(A.W, -A.R_lo), (double)A.nx);
+    const double R = __dadd_rn(A.R_lo, __dmul_rn(__dadd_rn((double)jr, 0.5), dR));
+    const double vt = __dmul_rn((double)kt, __ddiv_rn(3.14159265358979323846, (double)(A.ny - 1)));
+    double sv, cv;
+    sincos(vt, &sv, &cv);
+    alpha = __dmul_rn(R, cv);
+    beta = __dmul_rn(R, sv);
+  } else if (PIXELS == GRAY_PIXELS_GRID) {
     // pixel centres; explicit roundings so that (alpha, beta) are the same doubles on any machine
     const unsigned long long col = p % A.nx, row = p / A.nx;
     const double da = __ddiv_rn(__dmul_rn(2.0, A.W), (double)A.nx);
@@ -87,34 +97,38 @@ __global__ void __launch_bounds__(256) init_kernel(const __grid_constant__ InitA
 }
 
 static int init_common(gray_state* st, double a, double r_obs, double inc_deg, double W, int pixels,
-                       int32_t nx, int32_t ny, uint64_t seed, uint64_t p0, cudaStream_t stream) {
+                       int32_t nx, int32_t ny, uint64_t seed, uint64_t p0, cudaStream_t stream, double R_lo = 0.0) {
   int rc = check_state(st, false);
   if (rc) return rc;
   if (!(a > -1.0 && a < 1.0)) { set_error("spin a = %g outside (-1, 1)", a); return GRAY_ERR_DOMAIN; }
   if (!(r_obs > 0.0) || !(W > 0.0)) { set_error("r_obs and half_width must be positive"); return GRAY_ERR_DOMAIN; }
   if (!(inc_deg >= 0.0 && inc_deg <= 180.0)) { set_error("inclination %g outside [0, 180] degrees", inc_deg); return GRAY_ERR_DOMAIN; }
+  if (pixels == GRAY_PIXELS_POLAR && (!(R_lo >= 0.0 && R_lo < W) || ny < 2)) { set_error("polar grid needs 0 <= R_lo < R_hi and n_theta >= 2"); return GRAY_ERR_DOMAIN; }
   if (!(sqrt(r_obs * r_obs + 2.0 * W * W) < 1.01 * r_obs)) { set_error("half_width %g too large for r_obs %g: a pixel would start outside 1.01 r_obs", W, r_obs); return GRAY_ERR_DOMAIN; }
-  if (pixels == GRAY_PIXELS_GRID) {
+  if (pixels == GRAY_PIXELS_GRID || pixels == GRAY_PIXELS_POLAR) {
     if (nx <= 0 || ny <= 0) { set_error("nx, ny must be positive"); return GRAY_ERR_ARG; }
     if (p0 + st->n > (uint64_t)nx * (uint64_t)ny) { set_error("p0 + n = %llu exceeds nx * ny = %llu", (unsigned long long)(p0 + st->n), (unsigned long long)nx * ny); return GRAY_ERR_ARG; }
   }
   st->pixels = pixels;
   st->a = a; st->r_obs = r_obs; st->inc_deg = inc_deg; st->half_width = W;
-  st->nx = pixels == GRAY_PIXELS_GRID ? nx : 0;
-  st->ny = pixels == GRAY_PIXELS_GRID ? ny : 0;
-  st->seed = seed; st->p0 = p0;
+  st->nx = pixels != GRAY_PIXELS_RANDOM ? nx : 0;
+  st->ny = pixels != GRAY_PIXELS_RANDOM ? ny : 0;
+  st->seed = seed; st->p0 = p0; st->r_lo = R_lo;
   if (st->n == 0) return GRAY_OK;
   InitArgs A;
   A.x = st->x_dev; A.k = st->k_dev; A.status = st->status_dev; A.steps = st->steps_dev;
   A.n = st->n; A.p0 = p0; A.seed = seed;
-  A.a = a; A.r_obs = r_obs; A.W = W;
+  A.a = a; A.r_obs = r_obs; A.W = W; A.R_lo = R_lo;
   const double inc = inc_deg * 3.14159265358979323846 / 180.0;
   A.sin_i = sin(inc); A.cos_i = cos(inc);
   A.nx = (unsigned long long)(nx > 0 ? nx : 1); A.ny = (unsigned long long)(ny > 0 ? ny : 1);
   const unsigned long long blocks = (st->n + 255) / 256;
   if (blocks > 0x7fffffffull) { set_error("n too large"); return GRAY_ERR_ARG; }
   const bool f32 = st->prec == GRAY_F32;
-  if (pixels == GRAY_PIXELS_GRID) {
+  if (pixels == GRAY_PIXELS_POLAR) {
+    if (f32) init_kernel<float, GRAY_PIXELS_POLAR><<<(unsigned)blocks, 256, 0, stream>>>(A);
+    else init_kernel<double, GRAY_PIXELS_POLAR><<<(unsigned)blocks, 256, 0, stream>>>(A);
+  } else if (pixels == GRAY_PIXELS_GRID) {
     if (f32) init_kernel<float, GRAY_PIXELS_GRID><<<(unsigned)blocks, 256, 0, stream>>>(A);
     else init_kernel<double, GRAY_PIXELS_GRID><<<(unsigned)blocks, 256, 0, stream>>>(A);
   } else {
@@ -133,6 +147,12 @@ int gray_init_rays(gray_state* state, double a, double r_obs, double inc_deg, do
                    int32_t nx, int32_t ny, uint64_t p0, void* cuda_stream) {
   return gray::init_common(state, a, r_obs, inc_deg, half_width, GRAY_PIXELS_GRID, nx, ny, 0, p0,
                            (cudaStream_t)cuda_stream);
+}
+
+int gray_init_rays_polar(gray_state* state, double a, double r_obs, double inc_deg, double R_lo, double R_hi,
+                         int32_t n_R, int32_t n_theta, uint64_t p0, void* cuda_stream) {
+  return gray::init_common(state, a, r_obs, inc_deg, R_hi, GRAY_PIXELS_POLAR, n_R, n_theta, 0, p0,
+                           (cudaStream_t)cuda_stream, R_lo);
 }
 
 int gray_init_rays_random(gray_state* state, double a, double r_obs, double inc_deg, double half_width,

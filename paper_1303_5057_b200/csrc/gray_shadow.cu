@@ -151,6 +151,62 @@ __global__ void __launch_bounds__(1024) shadow_edge_kernel(const __grid_constant
   }
 }
 
+// Photon ring on the paper's polar grid (gray_ring_polar in gray.h; eqs. 6-10).  One block; a thread
+// per spoke walks inwards to the outermost captured cell, then eqs. (6)-(8) by block reductions (trapezoidal rule).
+struct RingArgs {
+  const uint8_t* status;
+  long long n_R, n_theta;
+  double R_lo, R_hi;
+  int bridge_axis;
+  double* radius;
+  Workspace* ws;
+};
+
+__device__ double ring_radius_raw(const RingArgs& A, long long k) {
+  const uint8_t* row = A.status + k * A.n_R;
+  long long j = A.n_R;
+  while (j > 0 && row[j - 1] != GRAY_CAPTURED) --j;      // outer edge of the outermost captured cell
+  return A.R_lo + (double)j * ((A.R_hi - A.R_lo) / (double)A.n_R);
+}
+__device__ double ring_radius(const RingArgs& A, long long k) {
+  if (A.bridge_axis && A.n_theta >= 3 && (A.n_theta % 2) == 1 && k == (A.n_theta - 1) / 2)
+    return 0.5 * (ring_radius_raw(A, k - 1) + ring_radius_raw(A, k + 1));      // the axis spoke (gray.h)
+  return ring_radius_raw(A, k);
+}
+
+__global__ void __launch_bounds__(1024) ring_polar_kernel(const __grid_constant__ RingArgs A) {
+  __shared__ double sh[32];
+  const double pi = 3.14159265358979323846;
+  const double amax = ring_radius(A, 0), amin = -ring_radius(A, A.n_theta - 1);
+  const double centre = (amin + amax) / 2.0;
+  const double step = pi / (double)(A.n_theta - 1);
+  auto R_of = [&](long long k, bool store) {
+    const double rho = ring_radius(A, k);
+    if (store && A.radius) A.radius[k] = rho;
+    double sv, cv;
+    sincos((double)k * step, &sv, &cv);
+    const double x = rho * cv - centre, y = rho * sv;
+    return sqrt(x * x + y * y);
+  };
+  double sum = 0.0;
+  for (long long k = threadIdx.x; k < A.n_theta; k += blockDim.x)
+    sum += ((k == 0 || k == A.n_theta - 1) ? 0.5 : 1.0) * R_of(k, true);
+  const double mean = block_sum(sum, sh) / (double)(A.n_theta - 1);
+  double var = 0.0;
+  for (long long k = threadIdx.x; k < A.n_theta; k += blockDim.x) {
+    const double d = R_of(k, false) - mean;
+    var += ((k == 0 || k == A.n_theta - 1) ? 0.5 : 1.0) * d * d;
+  }
+  var = block_sum(var, sh) / (double)(A.n_theta - 1);
+  if (threadIdx.x == 0) {
+    A.ws->stats[0] = amin;
+    A.ws->stats[1] = amax;
+    A.ws->stats[2] = fabs(amin + amax) / 2.0;
+    A.ws->stats[3] = mean;
+    A.ws->stats[4] = 2.0 * sqrt(var);
+  }
+}
+
 static unsigned int reduce_grid(unsigned long long n, unsigned long long per_thread) {
   unsigned long long blocks = (n / per_thread + 255) / 256 + 1;
   const unsigned long long cap = (unsigned long long)sm_count() * 16;
@@ -219,6 +275,34 @@ int gray_shadow_edge(const gray_state* state, int32_t n_angles, double* radius_d
   stats_host->alpha_min = s[3]; stats_host->alpha_max = s[4]; stats_host->D = s[5];
   stats_host->R_mean = s[6]; stats_host->A = s[7];
   stats_host->n_captured = ncap;
+  return GRAY_OK;
+}
+
+int gray_ring_polar(const gray_state* state, int32_t bridge_axis, double* radius_dev, gray_ring_stats* stats_host,
+                    void* workspace_dev, size_t workspace_bytes, void* cuda_stream) {
+  using namespace gray;
+  int rc = check_state(state, true);
+  if (rc) return rc;
+  if (!stats_host) { set_error("stats_host is NULL"); return GRAY_ERR_ARG; }
+  if (state->pixels != GRAY_PIXELS_POLAR || state->p0 != 0 || state->nx <= 0 || state->ny < 2 ||
+      state->n != (uint64_t)state->nx * (uint64_t)state->ny) {
+    set_error("gray_ring_polar needs a full polar image (pixels = POLAR, p0 = 0, n = n_R * n_theta)");
+    return GRAY_ERR_ARG;
+  }
+  rc = check_workspace(workspace_dev, workspace_bytes);
+  if (rc) return rc;
+  cudaStream_t stream = (cudaStream_t)cuda_stream;
+  Workspace* ws = (Workspace*)workspace_dev;
+  RingArgs A;
+  A.status = state->status_dev; A.n_R = state->nx; A.n_theta = state->ny;
+  A.R_lo = state->r_lo; A.R_hi = state->half_width; A.bridge_axis = bridge_axis; A.radius = radius_dev; A.ws = ws;
+  ring_polar_kernel<<<1, 1024, 0, stream>>>(A);
+  GRAY_CUDA(cudaGetLastError());
+  double s[5];
+  GRAY_CUDA(cudaMemcpyAsync(s, &ws->stats[0], sizeof s, cudaMemcpyDeviceToHost, stream));
+  GRAY_CUDA(cudaStreamSynchronize(stream));
+  stats_host->alpha_min = s[0]; stats_host->alpha_max = s[1]; stats_host->D = s[2];
+  stats_host->R_mean = s[3]; stats_host->A = s[4];
   return GRAY_OK;
 }
 

@@ -12,7 +12,7 @@ GRAY_F32, GRAY_F64 = 0, 1
 STEP_REL, STEP_EQ2 = 0, 1
 LIVE, CAPTURED, ESCAPED, BAD, EQUATOR = 0, 1, 2, 3, 4
 SCHED_REFILL, SCHED_STATIC = 0, 1
-PIXELS_GRID, PIXELS_RANDOM = 0, 1
+PIXELS_GRID, PIXELS_RANDOM, PIXELS_POLAR = 0, 1, 2
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB = None
@@ -26,7 +26,7 @@ class _State(C.Structure):
     _fields_ = [("x_dev", C.c_void_p), ("k_dev", C.c_void_p), ("status_dev", C.c_void_p), ("steps_dev", C.c_void_p),
                 ("n", C.c_uint64), ("prec", C.c_int32), ("pixels", C.c_int32), ("a", C.c_double),
                 ("r_obs", C.c_double), ("inc_deg", C.c_double), ("half_width", C.c_double), ("nx", C.c_int32),
-                ("ny", C.c_int32), ("seed", C.c_uint64), ("p0", C.c_uint64)]
+                ("ny", C.c_int32), ("seed", C.c_uint64), ("p0", C.c_uint64), ("r_lo", C.c_double)]
 
 
 class _StepParams(C.Structure):
@@ -39,6 +39,10 @@ class _StepParams(C.Structure):
 class _Counters(C.Structure):
     _fields_ = [("photon_steps", C.c_uint64), ("issued_steps", C.c_uint64), ("photons_done", C.c_uint64),
                 ("photons_live", C.c_uint64), ("fallback_steps", C.c_uint64)]
+
+
+class _RingStats(C.Structure):
+    _fields_ = [(k, C.c_double) for k in ("alpha_min", "alpha_max", "D", "R_mean", "A")]
 
 
 class _ShadowStats(C.Structure):
@@ -61,6 +65,8 @@ def lib():
         L = C.CDLL(path)
         vp, u64, i32, dbl = C.c_void_p, C.c_uint64, C.c_int32, C.c_double
         L.gray_init_rays.argtypes = [C.POINTER(_State), dbl, dbl, dbl, dbl, i32, i32, u64, vp]
+        L.gray_init_rays_polar.argtypes = [C.POINTER(_State), dbl, dbl, dbl, dbl, dbl, i32, i32, u64, vp]
+        L.gray_ring_polar.argtypes = [C.POINTER(_State), i32, vp, C.POINTER(_RingStats), vp, C.c_size_t, vp]
         L.gray_init_rays_random.argtypes = [C.POINTER(_State), dbl, dbl, dbl, dbl, u64, u64, vp]
         L.gray_workspace_bytes.argtypes = [u64]
         L.gray_workspace_bytes.restype = C.c_size_t
@@ -77,7 +83,7 @@ def lib():
         L.gray_device_info.argtypes = [C.POINTER(i32), C.POINTER(i32)]
         L.gray_last_error.restype = C.c_char_p
         L.gray_version.restype = C.c_char_p
-        for name in ("gray_init_rays", "gray_init_rays_random", "gray_integrate", "gray_integrate_counters",
+        for name in ("gray_init_rays", "gray_init_rays_random", "gray_init_rays_polar", "gray_ring_polar", "gray_integrate", "gray_integrate_counters",
                      "gray_classify", "gray_shadow_edge", "gray_fma_peak", "gray_packed_peak", "gray_device_info", "gray_integrate_host"):
             getattr(L, name).restype = C.c_int
         _LIB = L
@@ -121,7 +127,7 @@ class PhotonBatch:
         self.steps = torch.empty((self.n,), dtype=torch.int32, device=device)
         self.workspace = torch.zeros((gray_workspace_bytes(self.n),), dtype=torch.uint8, device=device)
         self.c = _State(self.x.data_ptr(), self.k.data_ptr(), self.status.data_ptr(), self.steps.data_ptr(),
-                        self.n, prec, 0, 0.0, 0.0, 0.0, 0.0, 0, 0, 0, 0)
+                        self.n, prec, 0, 0.0, 0.0, 0.0, 0.0, 0, 0, 0, 0, 0.0)
 
     def set_image_plane(self, a, r_obs, inc_deg, half_width, nx=0, ny=0, seed=0, p0=0, pixels=PIXELS_GRID):
         """Describe the image plane without running gray_init_rays (for states uploaded by the caller)."""
@@ -139,6 +145,18 @@ def gray_version():
 
 def gray_init_rays(batch, a, r_obs, inc_deg, half_width, nx, ny, p0=0):
     _check(lib().gray_init_rays(C.byref(batch.c), a, r_obs, inc_deg, half_width, nx, ny, p0, _stream()))
+
+
+def gray_init_rays_polar(batch, a, r_obs, inc_deg, R_lo, R_hi, n_R, n_theta, p0=0):
+    _check(lib().gray_init_rays_polar(C.byref(batch.c), a, r_obs, inc_deg, R_lo, R_hi, n_R, n_theta, p0, _stream()))
+
+
+def gray_ring_polar(batch, radius=None, bridge_axis=False):
+    """Returns the gray_ring_stats as a dict; fills radius (float64 tensor of n_theta) if given."""
+    s = _RingStats()
+    _check(lib().gray_ring_polar(C.byref(batch.c), int(bool(bridge_axis)), _ptr(radius), C.byref(s), _ptr(batch.workspace),
+                                 batch.workspace.numel(), _stream()))
+    return {k: getattr(s, k) for k, _ in _RingStats._fields_}
 
 
 def gray_init_rays_random(batch, a, r_obs, inc_deg, half_width, seed, p0=0):
