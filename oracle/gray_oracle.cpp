@@ -60,6 +60,14 @@ void gray_oracle_christoffel(double a, double r, double th, double* G64) {
 
 void gray_oracle_rhs(double a, const double* y, double* dy) { go::rhs(a, y, dy); }
 
+void gray_oracle_rhs_reduced(double a, double E, double L, const double* y6, double* dy6) {
+  go::rhs_reduced(a, E, L, y6, dy6);
+}
+
+void gray_oracle_killing_velocities(double a, double E, double L, double r, double th, double* kt, double* kp) {
+  go::killing_velocities(a, E, L, r, th, kt, kp);
+}
+
 void gray_oracle_invariants(double a, const double* y, double* inv4) { go::invariants(a, y, inv4); }
 
 void gray_oracle_pixel_grid(double W, int64_t nx, int64_t ny, uint64_t p, double* alpha, double* beta) {
@@ -90,8 +98,8 @@ void gray_oracle_remap_theta(double* y) { go::remap_theta(y); }
 // Integrate one ray from state y (in/out).  See gray_oracle::integrate.
 int gray_oracle_integrate(double a, double* y, double h, double r_capture, double r_escape, int rule,
                           uint32_t max_steps, int64_t force_steps, uint32_t* steps, double xi_eps,
-                          int stop_at_equator) {
-  go::StepParams sp{h, r_capture, r_escape, rule, xi_eps, stop_at_equator};
+                          int stop_at_equator, int system) {
+  go::StepParams sp{h, r_capture, r_escape, rule, xi_eps, stop_at_equator, system};
   return go::integrate(a, y, sp, max_steps, force_steps, steps);
 }
 
@@ -114,11 +122,11 @@ int gray_oracle_trace(double a, double r_obs, double inc_deg, double W, int64_t 
                       double esc_factor, double horizon_delta, int rule, uint32_t max_steps,
                       int init_f32, const int64_t* force_steps, int n_threads, double* y0_out,
                       double* y_out, int32_t* status_out, uint32_t* steps_out, double xi_eps, int stop_at_equator,
-                      double polar_R_lo) {
+                      double polar_R_lo, int system) {
   if (n_threads < 1) n_threads = 1;
   double rh = go::horizon(a);
   go::StepParams sp{h, cap_factor > 0 ? cap_factor * rh : rh + horizon_delta, esc_factor * r_obs, rule, xi_eps,
-                    stop_at_equator};
+                    stop_at_equator, system};
   double inc = inc_deg * kPi / 180.0;
   auto work = [&](uint64_t lo, uint64_t hi) {
     for (uint64_t j = lo; j < hi; ++j) {

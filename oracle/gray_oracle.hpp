@@ -44,6 +44,7 @@ namespace gray_oracle {
 
 enum Status : int { LIVE = 0, CAPTURED = 1, ESCAPED = 2, BAD = 3, EQUATOR = 4 };
 enum StepRule : int { STEP_REL = 0, STEP_EQ2 = 1 };
+enum System : int { SYS_FULL = 0, SYS_REDUCED = 1 };
 
 // ---------------------------------------------------------------- geometry
 // Kerr metric in Boyer-Lindquist coordinates (the spacetime of P:75; r_bh there
@@ -178,6 +179,57 @@ void invariants(T a, const T y[8], T inv[4]) {
   inv[0] = E; inv[1] = L; inv[2] = Q; inv[3] = norm / (g[0][0] * kt * kt);
 }
 
+// ------------------------------------------------------------ reduced system
+// NEXT-3 of SURVEY §8(f) (R0, R21).  The notation of the paper's eqs. (2) and (4) (dt/dlambda' and
+// dphi/dlambda' appear as velocities, the remap flips k_theta only) suggests that GRay itself integrates the system of
+// Psaltis & Johannsen (2012) in which the two Killing constants E = -k_t and L_z = k_phi are used to ELIMINATE k^t
+// and k^phi: t and phi obey first-order equations, r and theta second-order ones.  Written out from the metric:
+//   k^t   = -g^tt E + g^tphi L,   k^phi = -g^tphi E + g^phiphi L          (inverse Kerr metric, textbook)
+//         = (A E - 2 a r L) / (Sigma Delta),   (2 a r E + (Sigma - 2r) L / s^2) / (Sigma Delta),
+//           A = (r^2 + a^2)^2 - a^2 Delta s^2
+//   dr/dl = k^r, dtheta/dl = k^theta, and dk^r/dl, dk^theta/dl by the same Christoffel contraction as rhs(),
+//   evaluated with those k^t, k^phi.
+// State y6 = (t, r, theta, phi, k^r, k^theta); E and L are constants of the ray taken from its initial state.
+template <class T>
+void killing_velocities(T a, T E, T L, T r, T th, T* kt, T* kp) {
+  T s = sin(th);
+  T a2 = a * a, r2 = r * r, s2 = s * s;
+  T c = cos(th);
+  T Sigma = r2 + a2 * c * c;
+  T Delta = r2 - T(2) * r + a2;
+  T rho = r2 + a2;
+  T A = rho * rho - a2 * Delta * s2;
+  *kt = (A * E - T(2) * a * r * L) / (Sigma * Delta);
+  *kp = (T(2) * a * r * E + (Sigma - T(2) * r) * L / s2) / (Sigma * Delta);
+}
+
+template <class T>
+void rhs_reduced(T a, T E, T L, const T y6[6], T dy6[6]) {
+  T y[8], dy[8];
+  y[0] = y6[0]; y[1] = y6[1]; y[2] = y6[2]; y[3] = y6[3]; y[5] = y6[4]; y[6] = y6[5];
+  killing_velocities(a, E, L, y6[1], y6[2], &y[4], &y[7]);
+  rhs(a, y, dy);                        // dy[4], dy[7] (the equations that were eliminated) are not used
+  dy6[0] = y[4]; dy6[1] = y[5]; dy6[2] = y[6]; dy6[3] = y[7]; dy6[4] = dy[5]; dy6[5] = dy[6];
+}
+
+// One classical RK4 step of the reduced system on the full 8-component state: E, L are taken from y (invariants()),
+// the six evolving components are stepped, and k^t, k^phi of the result are rebuilt from the constants.
+template <class T>
+void rk4_step_reduced(T a, T E, T L, T y[8], T dl) {
+  T y6[6] = {y[0], y[1], y[2], y[3], y[5], y[6]};
+  T k1[6], k2[6], k3[6], k4[6], w[6];
+  rhs_reduced(a, E, L, y6, k1);
+  for (int i = 0; i < 6; ++i) w[i] = y6[i] + T(0.5) * dl * k1[i];
+  rhs_reduced(a, E, L, w, k2);
+  for (int i = 0; i < 6; ++i) w[i] = y6[i] + T(0.5) * dl * k2[i];
+  rhs_reduced(a, E, L, w, k3);
+  for (int i = 0; i < 6; ++i) w[i] = y6[i] + dl * k3[i];
+  rhs_reduced(a, E, L, w, k4);
+  for (int i = 0; i < 6; ++i) y6[i] = y6[i] + dl * (k1[i] + T(2) * k2[i] + T(2) * k3[i] + k4[i]) / T(6);
+  y[0] = y6[0]; y[1] = y6[1]; y[2] = y6[2]; y[3] = y6[3]; y[5] = y6[4]; y[6] = y6[5];
+  killing_velocities(a, E, L, y[1], y[2], &y[4], &y[7]);
+}
+
 // --------------------------------------------------------- image plane (O1-O3)
 // Pixel centres of an nx x ny grid over [-W, W]^2; photon index p = row*nx+col,
 // beta (row) slow.  ("grid spacing"; reading R1.)
@@ -296,7 +348,9 @@ struct StepParams {
   double r_escape;     // escaped  when r >  r_escape   (1.01 r_obs)
   int rule;            // StepRule
   double xi_eps = 0.0; // > 0: the paper's production pole treatment with epsilon = xi_eps, see integrate()
-  int stop_at_equator = 0;  // != 0: the grid-projection workload, see equator_hit()
+  int stop_at_equator = 0;  // != 0: the grid-projection workload, see equator_land()
+  int system = SYS_FULL;    // SYS_REDUCED: see rhs_reduced()
+  double E = 1.0, L = 0.0;  // SYS_REDUCED: constants of the ray being integrated (filled by integrate())
 };
 
 // Status of a state after a full step: non-finite -> BAD,
@@ -318,6 +372,10 @@ inline int classify_state(const double y[8], const StepParams& sp) {
 // the test.  One step (RK4 or its Euler replacement) counts as one step.
 inline void advance(double a, double y[8], const StepParams& sp, const double* forced_dl = nullptr) {
   double dl = forced_dl ? *forced_dl : step_size(a, y, sp.h, sp.rule);
+  if (sp.system == SYS_REDUCED) {         // E, L of the ray: carried by the caller in sp_E, sp_L (set by integrate())
+    rk4_step_reduced(a, sp.E, sp.L, y, dl);
+    return;
+  }
   if (!(sp.xi_eps > 0.0)) { rk4_step(a, y, dl); return; }
   double y_old[8], inv[4];
   for (int i = 0; i < 8; ++i) y_old[i] = y[i];
@@ -355,8 +413,14 @@ inline void equator_land(double a, double y[8], const StepParams& sp, uint32_t* 
 // step counter (in/out), so a call can resume an earlier one.  If force_steps >= 0 the tests are ignored and
 // exactly that many further steps are taken (the equal-step-count protocol, reading R11); the
 // returned status is then that of the last state.
-inline int integrate(double a, double y[8], const StepParams& sp, uint32_t max_steps,
+inline int integrate(double a, double y[8], const StepParams& sp_in, uint32_t max_steps,
                      int64_t force_steps, uint32_t* steps) {
+  StepParams sp = sp_in;
+  if (sp.system == SYS_REDUCED) {
+    double inv[4];
+    invariants(a, y, inv);
+    sp.E = inv[0]; sp.L = inv[1];
+  }
   if (force_steps >= 0) {
     for (int64_t n = 0; n < force_steps; ++n) {
       advance(a, y, sp);

@@ -11,6 +11,7 @@ from . import build as _build
 
 LIVE, CAPTURED, ESCAPED, BAD, EQUATOR = 0, 1, 2, 3, 4
 STEP_REL, STEP_EQ2 = 0, 1
+SYS_FULL, SYS_REDUCED = 0, 1
 
 _lib = None
 _dp = C.POINTER(C.c_double)
@@ -26,6 +27,8 @@ def lib():
         L.gray_oracle_metric.argtypes = [C.c_double] * 3 + [_dp]
         L.gray_oracle_christoffel.argtypes = [C.c_double] * 3 + [_dp]
         L.gray_oracle_rhs.argtypes = [C.c_double, _dp, _dp]
+        L.gray_oracle_rhs_reduced.argtypes = [C.c_double, C.c_double, C.c_double, _dp, _dp]
+        L.gray_oracle_killing_velocities.argtypes = [C.c_double] * 5 + [_dp, _dp]
         L.gray_oracle_invariants.argtypes = [C.c_double, _dp, _dp]
         L.gray_oracle_pixel_grid.argtypes = [C.c_double, C.c_int64, C.c_int64, C.c_uint64, _dp, _dp]
         L.gray_oracle_pixel_random.argtypes = [C.c_uint64, C.c_uint64, C.c_double, _dp, _dp]
@@ -37,13 +40,13 @@ def lib():
         L.gray_oracle_remap_theta.argtypes = [_dp]
         L.gray_oracle_integrate.restype = C.c_int
         L.gray_oracle_integrate.argtypes = [C.c_double, _dp, C.c_double, C.c_double, C.c_double, C.c_int,
-                                            C.c_uint32, C.c_int64, C.POINTER(C.c_uint32), C.c_double, C.c_int]
+                                            C.c_uint32, C.c_int64, C.POINTER(C.c_uint32), C.c_double, C.c_int, C.c_int]
         L.gray_oracle_trace.restype = C.c_int
         L.gray_oracle_trace.argtypes = [C.c_double] * 4 + [C.c_int64, C.c_int64, C.c_uint64, C.c_void_p,
                                                             C.c_uint64, C.c_double, C.c_double, C.c_double,
                                                             C.c_double, C.c_int, C.c_uint32, C.c_int,
                                                             C.c_void_p, C.c_int, C.c_void_p, C.c_void_p,
-                                                            C.c_void_p, C.c_void_p, C.c_double, C.c_int, C.c_double]
+                                                            C.c_void_p, C.c_void_p, C.c_double, C.c_int, C.c_double, C.c_int]
         L.gray_oracle_hardware_threads.restype = C.c_int
         L.gray_oracle_shadow_stats.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_double, C.c_int32,
                                                C.c_void_p, C.c_void_p]
@@ -81,6 +84,19 @@ def rhs(a, y):
     dy = np.zeros(8)
     lib().gray_oracle_rhs(a, y.ctypes.data_as(_dp), dy.ctypes.data_as(_dp))
     return dy
+
+
+def rhs_reduced(a, E, L, y6):
+    y6 = _vec(y6, 6)
+    dy = np.zeros(6)
+    lib().gray_oracle_rhs_reduced(a, E, L, y6.ctypes.data_as(_dp), dy.ctypes.data_as(_dp))
+    return dy
+
+
+def killing_velocities(a, E, L, r, th):
+    kt, kp = C.c_double(), C.c_double()
+    lib().gray_oracle_killing_velocities(a, E, L, r, th, C.byref(kt), C.byref(kp))
+    return kt.value, kp.value
 
 
 def invariants(a, y):
@@ -126,12 +142,13 @@ def remap_theta(y):
     return y
 
 
-def integrate(a, y, h, r_capture, r_escape, rule, max_steps, force_steps=-1, steps=0, xi_eps=0.0, stop_at_equator=False):
+def integrate(a, y, h, r_capture, r_escape, rule, max_steps, force_steps=-1, steps=0, xi_eps=0.0, stop_at_equator=False,
+              system=SYS_FULL):
     """Integrate one ray; returns (y, status, steps)."""
     y = _vec(y, 8).copy()
     st = C.c_uint32(steps)
     status = lib().gray_oracle_integrate(a, y.ctypes.data_as(_dp), h, r_capture, r_escape, rule, max_steps,
-                                         force_steps, C.byref(st), xi_eps, int(bool(stop_at_equator)))
+                                         force_steps, C.byref(st), xi_eps, int(bool(stop_at_equator)), system)
     return y, status, st.value
 
 
@@ -141,7 +158,7 @@ def hardware_threads():
 
 def trace(a, r_obs, inc_deg, W, nx=0, ny=0, seed=0, idx=None, n=None, h=1.0 / 32, cap_factor=1.01,
           esc_factor=1.01, horizon_delta=1e-6, rule=STEP_EQ2, max_steps=20000, init_f32=False,
-          force_steps=None, threads=1, want_y0=True, xi_eps=0.0, stop_at_equator=False, polar=None):
+          force_steps=None, threads=1, want_y0=True, xi_eps=0.0, stop_at_equator=False, polar=None, system=SYS_FULL):
     """Initialise and integrate a batch of photons; see gray_oracle_trace in gray_oracle.cpp.
     polar = (R_lo, R_hi, n_R, n_theta) selects the paper's polar image-plane grid (W, nx, ny are then ignored).
 
@@ -168,7 +185,7 @@ def trace(a, r_obs, inc_deg, W, nx=0, ny=0, seed=0, idx=None, n=None, h=1.0 / 32
                             horizon_delta, rule, max_steps, int(bool(init_f32)),
                             force_steps.ctypes.data if force_steps is not None else None, threads,
                             y0.ctypes.data if y0 is not None else None, y.ctypes.data,
-                            status.ctypes.data, steps.ctypes.data, xi_eps, int(bool(stop_at_equator)), R_lo)
+                            status.ctypes.data, steps.ctypes.data, xi_eps, int(bool(stop_at_equator)), R_lo, system)
     return dict(y0=y0, y=y, status=status, steps=steps)
 
 

@@ -346,3 +346,62 @@ def test_polar_ring_study_against_bardeen_and_paper_fits(a, inc):
     assert abs(st["A"] - ex["A"]) < dR
     Rf, Af = _paper_fit(a, inc)                                                # eqs. (11)-(14): soft, they are fits
     assert abs(st["R_mean"] - Rf) < 0.04 and abs(st["A"] - Af) < 0.04
+
+
+def _random_null_state(rng, a):
+    r, th = rng.uniform(2.5, 50.0), rng.uniform(0.2, np.pi - 0.2)
+    kr, kh, kp = rng.normal(size=3) * np.array([1.0, 1.0 / r, 1.0 / (r * np.sin(th))])
+    g = o.metric(a, r, th)
+    C = g[1, 1] * kr * kr + g[2, 2] * kh * kh + g[3, 3] * kp * kp
+    B = g[0, 3] * kp
+    kt = (-B - np.sqrt(B * B - g[0, 0] * C)) / g[0, 0]
+    return np.array([0.0, r, th, rng.uniform(-3, 3), kt, kr, kh, kp])
+
+
+def test_reduced_system_is_the_full_system_with_the_killing_constants_eliminated():
+    # NEXT-3.  Pin: the full right-hand side (itself pinned by the conservation laws): at any state, k^t and k^phi
+    # rebuilt from E = -k_t and L_z = k_phi are the state's own, and the r, theta accelerations coincide.
+    rng = np.random.default_rng(5)
+    for a in (0.0, 0.5, 0.99):
+        for _ in range(50):
+            y = _random_null_state(rng, a)
+            E, L, Q, _n = o.invariants(a, y)
+            kt, kp = o.killing_velocities(a, E, L, y[1], y[2])
+            assert abs(kt - y[4]) <= 1e-12 * abs(y[4]) and abs(kp - y[7]) <= 1e-12 * max(abs(y[7]), abs(y[4]) / y[1] ** 2)
+            d6 = o.rhs_reduced(a, E, L, y[[0, 1, 2, 3, 5, 6]])
+            d8 = o.rhs(a, y)
+            scale = np.abs(d8).max()
+            assert np.all(np.abs(d6 - d8[[0, 1, 2, 3, 5, 6]]) <= 1e-12 * np.maximum(np.abs(d8[[0, 1, 2, 3, 5, 6]]), scale * 1e-3))
+
+
+def test_reduced_system_integration_classifies_conserves_and_converges_to_the_full_system():
+    R = o.SYS_REDUCED
+    # a = 0: the sqrt(27) circle; Kerr: the exact radial-potential classifier
+    for a, inc, W in [(0.0, 60.0, 10.0), (0.9, 60.0, 10.0)]:
+        n = 24
+        res = o.trace(a, 1000.0, inc, W, n, n, rule=o.STEP_EQ2, threads=8, system=R)
+        al = -W + (np.arange(n) + 0.5) * 2 * W / n
+        A_, B_ = np.meshgrid(al, al)
+        rho_c = cf.bardeen_rho(a, inc, np.arctan2(B_, A_).ravel()) if a else np.full(n * n, np.sqrt(27.0))
+        band = np.abs(np.hypot(A_, B_).ravel() / rho_c - 1) < 0.01
+        inv = np.array([o.invariants(a, v) for v in res["y0"]])
+        exact = np.array([cf.captured_exact(a, L / E, Q / E ** 2) for E, L, Q, _ in inv])
+        assert np.all(((res["status"] == o.CAPTURED) == exact) | band)
+        inv1 = np.array([o.invariants(a, v) for v in res["y"]])
+        esc = res["status"] == o.ESCAPED
+        # E and L_z are constants of the reduced system: conserved to rounding, not to truncation
+        assert np.max(np.abs(inv1[esc, 0] - inv[esc, 0])) < 1e-12 and np.max(np.abs(inv1[esc, 1] - inv[esc, 1])) < 1e-11
+        assert np.max(np.abs(inv1[esc, 2] - inv[esc, 2]) / np.maximum(np.abs(inv[esc, 2]), 0.1)) < 1e-4      # Q: truncation
+    # step halving: Q drift and the distance to the full system's solution both fall ~16x per halving
+    a = 0.9
+    y0 = o.init_ray(a, 1000.0, 60.0, 6.0, 5.0)
+    Q0 = o.invariants(a, y0)[2]
+    dq, dist = [], []
+    for h in (1 / 16, 1 / 32, 1 / 64):
+        nsteps = int(round(300 * (1 / 16) / h))
+        yr = o.integrate(a, y0, h, 1.0, 1e9, o.STEP_REL, 10 ** 6, force_steps=nsteps, system=R)[0]
+        yf = o.integrate(a, y0, h, 1.0, 1e9, o.STEP_REL, 10 ** 6, force_steps=nsteps)[0]
+        dq.append(abs(o.invariants(a, yr)[2] - Q0))
+        dist.append(np.max(np.abs(yr[1:4] - yf[1:4])))
+    assert 10 < dq[0] / dq[1] < 40 and 10 < dq[1] / dq[2] < 40, dq                 # 4th order or better
+    assert 10 < dist[0] / dist[1] < 40 and 10 < dist[1] / dist[2] < 40, dist
