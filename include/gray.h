@@ -59,6 +59,14 @@ typedef enum { GRAY_F32 = 0, GRAY_F64 = 1 } gray_prec;
  *                  paper eq. (2), with its Delta := h ~ 1/32                          */
 typedef enum { GRAY_STEP_REL = 0, GRAY_STEP_EQ2 = 1 } gray_step_rule;
 
+/* Which equations gray_integrate advances (R0, R21).
+ *   GRAY_SYS_FULL     all eight: dx^mu/dl = k^mu, dk^mu/dl = -Gamma^mu_ab k^a k^b                  (BASELINE north_star)
+ *   GRAY_SYS_REDUCED  the Killing constants E = -k_t and L = k_phi, taken from the photon's state when it is
+ *                     loaded, eliminate k^t and k^phi: t and phi obey first-order equations with k^t, k^phi from
+ *                     the inverse metric, r and theta the same second-order ones (what the paper's own notation
+ *                     suggests GRay integrates).  The stored state keeps all eight components.  */
+typedef enum { GRAY_SYS_FULL = 0, GRAY_SYS_REDUCED = 1 } gray_system;
+
 typedef enum { GRAY_LIVE = 0, GRAY_CAPTURED = 1, GRAY_ESCAPED = 2, GRAY_BAD = 3,
                GRAY_EQUATOR = 4 /* reached theta = pi/2 (stop_at_equator only) */ } gray_ray_status;
 
@@ -150,6 +158,8 @@ typedef struct {
                                 re-integrated from the old state as ONE forward Euler step of dlambda / 9,
                                 which is not tested itself (reading R18).  0 = off.  Not available
                                 together with `frozen`.                                               */
+  int32_t system;            /* gray_system; GRAY_SYS_REDUCED excludes frozen, stop_at_equator, xi_epsilon  */
+  int32_t reserved;          /* must be 0                                                             */
 } gray_step_params;
 
 /* Bytes of device workspace gray_integrate / gray_classify / gray_shadow_edge need (queue head and

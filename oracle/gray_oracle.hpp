@@ -29,6 +29,8 @@
 //   equatorial projection : a = 0 line of nodes and orbit integral (phi, r at the
 //                           crossing to 2e-6); Kerr: invariants at the landed state,
 //                           reflection symmetry
+//   reduced system        : killing_velocities / rhs_reduced against the full rhs;
+//                           classifiers; E, L_z to rounding; step halving
 //   polar grid, ring stats: exact disc; Bardeen curve sampled on the same spokes;
 //                           the paper's fits eqs. 11-14 (soft)
 //   shadow statistics     : Bardeen closed-form curve (area, alpha extent, D,

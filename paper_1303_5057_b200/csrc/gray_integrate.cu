@@ -27,6 +27,7 @@ struct IntegrateArgs {
   uint32_t max_steps;
   int refill_interval;
   int stop_eq;               // gray_step_params.stop_at_equator
+  int reduced;               // gray_step_params.system == GRAY_SYS_REDUCED
   Workspace* ws;
   Consts<V> K;
 };
@@ -49,7 +50,7 @@ __device__ __forceinline__ unsigned long long warp_sum(unsigned long long v) {
   return v;
 }
 
-template <typename V, int RULE, int SCHED, bool FROZEN, bool XI, bool EQ>
+template <typename V, int RULE, int SCHED, bool FROZEN, bool XI, bool EQ, bool RED>
 __global__ void __launch_bounds__(kBlock, Tune<V>::min_blocks)
 integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
   using S = typename VT<V>::S;
@@ -98,6 +99,14 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
       ys[4][l] = kv.x; ys[5][l] = kv.y; ys[6][l] = kh; ys[7][l] = kv.w;
 #pragma unroll
       for (int i = 0; i < 8; ++i) cs[i][l] = S(0);
+      if (RED) {
+        // reduced system: the slots of k^t, k^phi carry the constants E, L of the photon, their compensation
+        // slots -a E, -a L (rk4_step_reduced)
+        S E, L;
+        killing_constants(vget(K.a, 0), vget(K.rp, 0), ys[1][l], th, kv.x, kv.w, E, L);
+        ys[4][l] = E; ys[7][l] = L;
+        cs[4][l] = vneg(vmul(vget(K.a, 0), E)); cs[7][l] = vneg(vmul(vget(K.a, 0), L));
+      }
       mirrored[l] = m;
       idx[l] = p;
       nst[l] = nst0[l] = iss[l] = s;
@@ -114,6 +123,7 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
     const S th = vget(y[2], l), kh = vget(y[6], l);
     xv.x = vget(y[0], l); xv.y = vget(y[1], l) + vget(K.rp, 0); xv.z = mirrored[l] ? pi_minus(th) : th; xv.w = vget(y[3], l);
     kv.x = vget(y[4], l); kv.y = vget(y[5], l); kv.z = mirrored[l] ? sneg(kh) : kh; kv.w = vget(y[7], l);
+    if (RED) killing_velocities(vget(K.a, 0), vget(K.rp, 0), vget(K.rpm, 0), vget(y[1], l), th, vget(y[4], l), vget(y[7], l), kv.x, kv.w);
     const unsigned long long p = idx[l];
     A.x[p] = xv;
     A.k[p] = kv;
@@ -164,7 +174,7 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
 #pragma unroll
       for (int l = 0; l < N; ++l) any |= have[l];
       if (any) {
-        V dl = step_size<V, RULE>(K, y[1], y[5], y[6], y[7]);
+        V dl = RED ? K.zero : step_size<V, RULE>(K, y[1], y[5], y[6], y[7]);
         if (EQ && lnd) {
           // landing on the equatorial plane: a Newton step dlambda = -(theta - pi/2) / k^theta instead of the rule
           S dls[N], ths[N], khs[N];
@@ -176,12 +186,13 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
         }
         if (!FROZEN) {
           bool rej[N];
-          rk4_step<XI>(K, y, comp, dl, rej);
+          if (RED) rk4_step_reduced<RULE>(K, y, comp);
+          else rk4_step<XI>(K, y, comp, dl, rej);
           if (XI) {
 #pragma unroll
             for (int l = 0; l < N; ++l) c_fallback += (rej[l] && have[l]) ? 1u : 0u;
           }
-          const V z = nonfinite_probe(K, y);
+          const V z = RED ? vfma(K.zero, y[6], vmul(K.zero, y[5])) : nonfinite_probe(K, y);
           const V r = vadd(y[1], K.rp);
           // Bookkeeping.  Common case first, with one branch for the whole thread: every slot's theta still in
           // [0, pi/2] (no eq. (3) remap, no fold) and no slot finished.
@@ -295,9 +306,9 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
   }
 }
 
-template <typename V, int RULE, int SCHED, bool FROZEN, bool XI, bool EQ>
+template <typename V, int RULE, int SCHED, bool FROZEN, bool XI, bool EQ, bool RED = false>
 static int launch(const IntegrateArgs<V>& A, cudaStream_t stream) {
-  auto kern = integrate_kernel<V, RULE, SCHED, FROZEN, XI, EQ>;
+  auto kern = integrate_kernel<V, RULE, SCHED, FROZEN, XI, EQ, RED>;
   constexpr unsigned long long per_block = (unsigned long long)kBlock * VT<V>::N;
   unsigned long long blocks_needed = (A.n + per_block - 1) / per_block;
   unsigned int grid;
@@ -318,6 +329,7 @@ static int launch(const IntegrateArgs<V>& A, cudaStream_t stream) {
 
 template <typename V, int RULE, int SCHED>
 static int dispatch_frozen(const IntegrateArgs<V>& A, bool frozen, cudaStream_t s) {
+  if (A.reduced) return launch<V, RULE, SCHED, false, false, false, true>(A, s);
   if (frozen) return launch<V, RULE, SCHED, true, false, false>(A, s);
   if (A.stop_eq) return A.K.xi_eps > 0 ? launch<V, RULE, SCHED, false, true, true>(A, s) : launch<V, RULE, SCHED, false, false, true>(A, s);
   return A.K.xi_eps > 0 ? launch<V, RULE, SCHED, false, true, false>(A, s) : launch<V, RULE, SCHED, false, false, false>(A, s);
@@ -341,6 +353,7 @@ static int integrate(const gray_state* st, uint64_t n, uint32_t max_steps, const
   A.max_steps = max_steps;
   A.refill_interval = p->refill_interval > 0 ? p->refill_interval : 8;
   A.stop_eq = p->stop_at_equator != 0;
+  A.reduced = p->system == GRAY_SYS_REDUCED;
   const double a = st->a, rh = 1.0 + sqrt(1.0 - a * a);
   A.K = make_consts<V>(a, p->h, p->r_capture_factor > 0.0 ? p->r_capture_factor * rh : rh + p->horizon_delta,
                        p->r_escape_factor * st->r_obs, p->xi_epsilon);
@@ -367,6 +380,11 @@ int gray_integrate(gray_state* state, uint64_t n_photons, uint32_t max_steps, co
   if (!(params->xi_epsilon >= 0.0)) { set_error("xi_epsilon must be >= 0"); return GRAY_ERR_DOMAIN; }
   if (params->xi_epsilon > 0.0 && params->frozen) { set_error("xi_epsilon > 0 is not available together with frozen"); return GRAY_ERR_UNSUPPORTED; }
   if (params->stop_at_equator && params->frozen) { set_error("stop_at_equator is not available together with frozen"); return GRAY_ERR_UNSUPPORTED; }
+  if (params->system != GRAY_SYS_FULL && params->system != GRAY_SYS_REDUCED) { set_error("bad system %d", params->system); return GRAY_ERR_ARG; }
+  if (params->system == GRAY_SYS_REDUCED && (params->frozen || params->stop_at_equator || params->xi_epsilon > 0.0)) {
+    set_error("the reduced system is not available together with frozen, stop_at_equator or xi_epsilon");
+    return GRAY_ERR_UNSUPPORTED;
+  }
   if (params->photons_per_thread < 0 || params->photons_per_thread > 2) { set_error("photons_per_thread must be 0 (default), 1 or 2"); return GRAY_ERR_ARG; }
   if (params->photons_per_thread == 2 && state->prec != GRAY_F32) { set_error("photons_per_thread = 2 (packed FP32 instructions) needs GRAY_F32"); return GRAY_ERR_UNSUPPORTED; }
   if (!(params->h > 0.0) || !(params->r_escape_factor > 0.0) || params->r_capture_factor < 0.0 ||

@@ -294,6 +294,128 @@ GRAY_DEV void rk4_step(const Consts<V>& K, V y[8], V comp[8], V dl, bool rejecte
   for (int i = 0; i < 8; ++i) { y[i] = yn[i]; comp[i] = cn[i]; }
 }
 
+// ======================================================================================================
+// Reduced system (NEXT-3; R21): the Killing constants E = -k_t, L = k_phi eliminate k^t and k^phi.
+//   u = k^t - a s^2 k^phi = (rho E - a L)/Delta,    w = Sigma k^phi - a u = L/s^2 - a E,
+//   k^phi = (w + a u)/Sigma,                        k^t = u + a s^2 k^phi
+// (the inverse Kerr metric applied to (-E, L), regrouped), and dk^r/dl, dk^theta/dl are the same expressions as
+// in geodesic_accel.  51 FP-pipe operations besides the sincos, against 66.
+// ======================================================================================================
+GRAY_DEV void sincos_s(float x, float& s, float& c) { sincosf(x, &s, &c); }
+GRAY_DEV void sincos_s(double x, double& s, double& c) { sincos(x, &s, &c); }
+
+// E, L of a stored state (scalar, once per photon on load)
+template <typename S>
+GRAY_DEV void killing_constants(S a, S rp, S d, S th, S kt, S kp, S& E, S& L) {
+  S s, c;
+  sincos_s(th, s, c);
+  const S r = vadd(d, rp);
+  const S r2 = vmul(r, r), s2 = vmul(s, s);
+  const S Sg = vfma(vmul(a, a), vmul(c, c), r2);
+  const S rho = vfma(a, a, r2);
+  const S f = vmul(vadd(r, r), vrcp_exact(Sg));                  // 2r/Sigma
+  const S af = vmul(a, f);
+  // E = (1 - 2r/Sigma) k^t + (2 a r s^2/Sigma) k^phi;  L = s^2 [(rho + a s^2 (2 a r/Sigma)) k^phi - (2 a r/Sigma) k^t]
+  E = vfma(vmul(af, s2), kp, vfma(vneg(f), kt, kt));
+  L = vmul(s2, vfma(vfma(vmul(a, s2), af, rho), kp, vneg(vmul(af, kt))));
+}
+// k^t, k^phi of a state from its constants (scalar, once per photon on retirement)
+template <typename S>
+GRAY_DEV void killing_velocities(S a, S rp, S rpm, S d, S th, S E, S L, S& kt, S& kp) {
+  S s, c;
+  sincos_s(th, s, c);
+  const S r = vadd(d, rp);
+  const S r2 = vmul(r, r), s2 = vmul(s, s);
+  const S Sg = vfma(vmul(a, a), vmul(c, c), r2);
+  const S rho = vfma(a, a, r2);
+  const S Dl = vmul(d, vadd(d, rpm));
+  const S u = vmul(vfma(rho, E, vneg(vmul(a, L))), vrcp_exact(Dl));
+  const S w = vfma(L, vrcp_exact(s2), vneg(vmul(a, E)));
+  kp = vmul(vfma(a, u, w), vrcp_exact(Sg));
+  kt = vfma(vmul(a, s2), kp, u);
+}
+
+// accelerations of (k^r, k^theta) -> out[0], out[1] (ACC: added to add[0], add[1]); k^t, k^phi of the point -> kt, kp
+template <bool ACC, typename V>
+GRAY_DEV void geodesic_accel_reduced(const Consts<V>& K, V d, V th, V kr, V kh, V E, V L, V naE, V naL, const V* add,
+                                     V out[2], V& kt, V& kp) {
+  V s, c;
+  sincos_v(K, th, s, c);
+  const V r = vadd(d, K.rp);
+  const V r2 = vmul(r, r);
+  const V c2 = vmul(c, c);
+  const V Sg = vfma(K.a2, c2, r2);
+  const V P = vfma(K.na2, c2, r2);
+  const V rho = vadd(r2, K.a2);
+  const V Dl = vmul(d, vadd(d, K.rpm));
+  const V iS = vrcp(Sg), iD = vrcp(Dl), is = vrcp(s);
+  const V niS = vneg(iS);
+  const V s2 = vmul(s, s);
+  const V sc = vmul(s, c);
+  const V u = vmul(vfma(rho, E, naL), iD);
+  const V w = vfma(L, vmul(is, is), naE);
+  kp = vmul(vfma(K.a, u, w), iS);
+  kt = vfma(vmul(K.a, s2), kp, u);
+  const V krD = vmul(kr, iD);
+  const V niS2 = vmul(iS, niS);
+  const V tiS2 = vadd(niS2, niS2);
+  const V Pu = vmul(P, u);
+  const V tk = vmul(sc, kh);
+  // dk^r
+  const V krkr = vmul(kr, kr);
+  const V G = vfma(vadd(d, K.rpm1), iD, vmul(r, niS));
+  const V kp2 = vmul(kp, kp), kh2 = vmul(kh, kh);
+  const V rA1 = vmul(r, vfma(s2, kp2, kh2));
+  const V Bp = vfma(vmul(Pu, u), niS2, rA1);
+  const V J2 = vfma(K.twoa2, vmul(tk, kr), vmul(Dl, Bp));
+  out[0] = vfma(krkr, G, ACC ? vfma(iS, J2, add[0]) : vmul(iS, J2));
+  // dk^theta
+  const V a2z1 = vfma(K.na2, vmul(krD, kr), vmul(K.a2, kh2));
+  const V z2 = vfma(Dl, kp2, a2z1);
+  const V z3 = vfma(vmul(r, vmul(w, w)), vneg(tiS2), z2);
+  const V z5 = vfma(K.m2, vmul(vmul(r, kr), kh), vmul(sc, z3));
+  out[1] = ACC ? vfma(iS, z5, add[1]) : vmul(iS, z5);
+}
+
+// One RK4 step of the reduced system.  y[4], y[7] hold the constants E, L of the photon and comp[4], comp[7] hold
+// -a E, -a L; neither is touched.  The step size (which needs k^phi) is formed after the first evaluation.
+template <int RULE, typename V>
+GRAY_DEV void rk4_step_reduced(const Consts<V>& K, V y[8], V comp[8]) {
+  const V E = y[4], L = y[7], naE = comp[4], naL = comp[7];
+  V f[2], kt, kp, acc[8], w1, w2, w5, w6;
+  geodesic_accel_reduced<false>(K, y[1], y[2], y[5], y[6], E, L, naE, naL, (const V*)nullptr, f, kt, kp);
+  const V dl = step_size<V, RULE>(K, y[1], y[5], y[6], kp);
+  const V hdl = vmul(K.half, dl);
+  acc[0] = kt; acc[3] = kp; acc[1] = y[5]; acc[2] = y[6]; acc[5] = f[0]; acc[6] = f[1];
+  w1 = vfma(hdl, y[5], y[1]); w2 = vfma(hdl, y[6], y[2]); w5 = vfma(hdl, f[0], y[5]); w6 = vfma(hdl, f[1], y[6]);
+#pragma unroll
+  for (int stage = 2; stage <= 3; ++stage) {
+    const V hs = stage == 2 ? hdl : dl;
+    geodesic_accel_reduced<false>(K, w1, w2, w5, w6, E, L, naE, naL, (const V*)nullptr, f, kt, kp);
+    acc[0] = vfma(K.two, kt, acc[0]); acc[3] = vfma(K.two, kp, acc[3]);
+    acc[1] = vfma(K.two, w5, acc[1]); acc[2] = vfma(K.two, w6, acc[2]);
+    acc[5] = vfma(K.two, f[0], acc[5]); acc[6] = vfma(K.two, f[1], acc[6]);
+    const V k5 = w5, k6 = w6;
+    w1 = vfma(hs, k5, y[1]); w2 = vfma(hs, k6, y[2]); w5 = vfma(hs, f[0], y[5]); w6 = vfma(hs, f[1], y[6]);
+  }
+  acc[1] = vadd(acc[1], w5); acc[2] = vadd(acc[2], w6);
+  geodesic_accel_reduced<true>(K, w1, w2, w5, w6, E, L, naE, naL, acc + 5, acc + 5, kt, kp);
+  acc[0] = vadd(acc[0], kt); acc[3] = vadd(acc[3], kp);
+  const V dl6 = vmul(K.sixth, dl);
+#pragma unroll
+  for (int i = 0; i < 7; ++i) {
+    if (i == 4) continue;
+    if (sizeof(typename VT<V>::S) == 4 && ((GRAY_COMP_MASK >> i) & 1)) {
+      const V inc = vfma(dl6, acc[i], comp[i]);
+      const V s = vadd(y[i], inc);
+      comp[i] = vsub(inc, vsub(s, y[i]));
+      y[i] = s;
+    } else {
+      y[i] = vfma(dl6, acc[i], y[i]);
+    }
+  }
+}
+
 // pi and 2 pi minus x with pi split in two parts of the working precision
 GRAY_DEV float pi_minus(float x) { return __fsub_rn(__fsub_rn(3.14159274101257324219f, x), 8.742278000372485e-08f); }
 GRAY_DEV double pi_minus(double x) { return (3.141592653589793116 - x) + 1.2246467991473532e-16; }

@@ -112,6 +112,10 @@ GRAY_DEV float vrcp(float x) { return srcp(x); }
 GRAY_DEV double vrcp(double x) { return __drcp_rn(x); }
 GRAY_DEV f2 vrcp(f2 v) { float lo, hi; f2_unpack(v, lo, hi); return f2_pack(srcp(lo), srcp(hi)); }
 
+// exact (IEEE) reciprocal for the scalar once-per-photon work of the reduced system
+GRAY_DEV float vrcp_exact(float x) { return __frcp_rn(x); }
+GRAY_DEV double vrcp_exact(double x) { return __drcp_rn(x); }
+
 // ---- min / max (ALU pipe for float) --------------------------------------------------------------------
 GRAY_DEV float vmax(float a, float b) { return fmaxf(a, b); }
 GRAY_DEV double vmax(double a, double b) { return fmax(a, b); }

@@ -10,6 +10,7 @@ import torch
 
 GRAY_F32, GRAY_F64 = 0, 1
 STEP_REL, STEP_EQ2 = 0, 1
+SYS_FULL, SYS_REDUCED = 0, 1
 LIVE, CAPTURED, ESCAPED, BAD, EQUATOR = 0, 1, 2, 3, 4
 SCHED_REFILL, SCHED_STATIC = 0, 1
 PIXELS_GRID, PIXELS_RANDOM, PIXELS_POLAR = 0, 1, 2
@@ -33,7 +34,7 @@ class _StepParams(C.Structure):
     _fields_ = [("h", C.c_double), ("r_capture_factor", C.c_double), ("horizon_delta", C.c_double),
                 ("r_escape_factor", C.c_double), ("rule", C.c_int32), ("schedule", C.c_int32),
                 ("refill_interval", C.c_int32), ("frozen", C.c_int32), ("photons_per_thread", C.c_int32),
-                ("stop_at_equator", C.c_int32), ("xi_epsilon", C.c_double)]
+                ("stop_at_equator", C.c_int32), ("xi_epsilon", C.c_double), ("system", C.c_int32), ("reserved", C.c_int32)]
 
 
 class _Counters(C.Structure):
@@ -107,9 +108,10 @@ class StepParams:
     """gray_step_params (include/gray.h).  Defaults: the BASELINE configs' h, capture and escape radii."""
 
     def __init__(self, h=1.0 / 32, r_capture_factor=1.01, horizon_delta=1e-6, r_escape_factor=1.01, rule=STEP_EQ2,
-                 schedule=SCHED_REFILL, refill_interval=0, frozen=False, photons_per_thread=0, xi_epsilon=0.0, stop_at_equator=False):
+                 schedule=SCHED_REFILL, refill_interval=0, frozen=False, photons_per_thread=0, xi_epsilon=0.0, stop_at_equator=False,
+                 system=SYS_FULL):
         self.c = _StepParams(h, r_capture_factor, horizon_delta, r_escape_factor, rule, schedule, refill_interval,
-                             int(bool(frozen)), photons_per_thread, int(bool(stop_at_equator)), xi_epsilon)
+                             int(bool(frozen)), photons_per_thread, int(bool(stop_at_equator)), xi_epsilon, system, 0)
 
 
 class PhotonBatch:
