@@ -104,8 +104,40 @@ GRAY_DEV void sincos_v(const Consts<V>& K, V x, V& s, V& c) {
     vset(c, l, cl);
   }
 }
+// double build, same scheme: quadrant by the magic constant 1.5 * 2^52, two-term Cody-Waite reduction (exact for the
+// |j| <= 2 that occur), Taylor polynomials to r^17 / r^16 on [-pi/4, pi/4] (truncation < 1e-18), Horner in FMAs:
+// 22 FP64-pipe operations, no slow path, against ~40 plus a Payne-Hanek branch in the CUDA library's sincos.
 template <>
-GRAY_DEV void sincos_v<double>(const Consts<double>&, double x, double& s, double& c) { sincos(x, &s, &c); }
+GRAY_DEV void sincos_v<double>(const Consts<double>&, double x, double& s, double& c) {
+  const double magic = 6755399441055744.0;
+  const double q = __fma_rn(x, 0.63661977236758134308, magic);
+  const int j = __double2loint(q);
+  const double jf = __dsub_rn(q, magic);
+  double r = __fma_rn(jf, -1.57079632679489655800e+00, x);
+  r = __fma_rn(jf, -6.12323399573676603587e-17, r);
+  const double u = __dmul_rn(r, r);
+  double sp = -7.6471637318198164759e-13;                       // -1/15!
+  sp = __fma_rn(sp, u, 1.6059043836821614599e-10);              //  1/13!
+  sp = __fma_rn(sp, u, -2.5052108385441718775e-08);             // -1/11!
+  sp = __fma_rn(sp, u, 2.7557319223985890653e-06);              //  1/9!
+  sp = __fma_rn(sp, u, -1.9841269841269841270e-04);             // -1/7!
+  sp = __fma_rn(sp, u, 8.3333333333333332177e-03);              //  1/5!
+  sp = __fma_rn(sp, u, -1.6666666666666665741e-01);             // -1/3!
+  const double sn = __fma_rn(__dmul_rn(r, u), sp, r);
+  double cp = 4.7794773323873852974e-14;                        //  1/16!
+  cp = __fma_rn(cp, u, -1.1470745597729724714e-11);             // -1/14!
+  cp = __fma_rn(cp, u, 2.0876756987868098979e-09);              //  1/12!
+  cp = __fma_rn(cp, u, -2.7557319223985888276e-07);             // -1/10!
+  cp = __fma_rn(cp, u, 2.4801587301587301566e-05);              //  1/8!
+  cp = __fma_rn(cp, u, -1.3888888888888889419e-03);             // -1/6!
+  cp = __fma_rn(cp, u, 4.1666666666666664354e-02);              //  1/4!
+  cp = __fma_rn(cp, u, -0.5);
+  const double cs = __fma_rn(u, cp, 1.0);
+  const bool swap = (j & 1) != 0;
+  const double ss = swap ? cs : sn, cc = swap ? sn : cs;
+  s = (j & 2) ? -ss : ss;                                       // quadrants 2, 3: sin < 0
+  c = ((j + 1) & 2) ? -cc : cc;                                 // quadrants 1, 2: cos < 0
+}
 
 // ---- right-hand side: accelerations dk^mu/dlambda at (d = r - r_+, th) for momentum (kt, kr, kh, kp) ----
 // out[i] = dk^i/dlambda (i = t, r, th, phi) if !ACC, else add[i] + dk^i/dlambda with the addition fused into the
