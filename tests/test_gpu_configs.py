@@ -43,7 +43,7 @@ def _gather(batch, idx):
 
 @pytest.mark.parametrize("log2n", [28, 30])
 def test_c4_throughput_workload_full_size_sampled(log2n):
-    # C4 realistic case exactly as bench.py runs it (2^28 is its default workload, 2^30 the north-star size):
+    # C4 realistic case exactly as bench.py runs it (2^30, the north-star size, is its default workload):
     # seeded random pixels, eq. (2) rule, lane refill, packed fp32 kernel.  4096 strided rays against the oracle.
     c4 = wl.C4
     n = 2 ** log2n
