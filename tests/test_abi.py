@@ -59,6 +59,21 @@ def test_argument_errors_are_reported_before_any_launch(libpath):
     sp = g.StepParams().c
     st.n = 0
     assert L.gray_integrate(ctypes.byref(st), 0, 10, ctypes.byref(sp), None, 0, None) == -3    # GRAY_ERR_WORKSPACE
+    # option combinations that have no kernel are refused by name, not approximated
+    for kw, code in ((dict(frozen=True, xi_epsilon=1e-3), -5), (dict(frozen=True, stop_at_equator=True), -5),
+                     (dict(system=g.SYS_REDUCED, xi_epsilon=1e-3), -5), (dict(system=g.SYS_REDUCED, frozen=True), -5),
+                     (dict(system=g.SYS_REDUCED, stop_at_equator=True), -5), (dict(xi_epsilon=-1.0), -2),
+                     (dict(system=7), -1), (dict(photons_per_thread=3), -1), (dict(rule=9), -1), (dict(schedule=5), -1)):
+        sp = g.StepParams(**kw).c
+        assert L.gray_integrate(ctypes.byref(st), 0, 10, ctypes.byref(sp), None, 0, None) == code, kw
+    st.prec = g.GRAY_F64
+    sp = g.StepParams(photons_per_thread=2).c
+    assert L.gray_integrate(ctypes.byref(st), 0, 10, ctypes.byref(sp), None, 0, None) == -5   # packed FP32 needs GRAY_F32
+    st.prec = g.GRAY_F32
+    assert L.gray_init_rays_polar(ctypes.byref(st), 0.5, 1000.0, 60.0, 7.5, 1.5, 10, 5, 0, None) == -2      # R_lo >= R_hi
+    assert L.gray_init_rays_polar(ctypes.byref(st), 0.5, 1000.0, 60.0, 1.5, 7.5, 10, 1, 0, None) == -2      # n_theta < 2
+    v = ctypes.c_double()
+    assert L.gray_packed_peak(3, 16, ctypes.byref(v), None) == -1 and L.gray_fma_peak(2, 16, ctypes.byref(v), None) == -1
 
 
 def test_product_does_not_import_the_oracle():
