@@ -31,10 +31,9 @@ FLOPS_PER_PHOTON_STEP = {"rel": 777, "eq2": 787}
 # FP32 CUDA-core peak the integrator is bound by: 148 SMs x 128 lanes x 2 (FMA) x
 # 1.965 GHz (clocks.max.sm); FP64: 64 lanes per SM.
 PEAK_TFLOPS = {"f32": 148 * 128 * 2 * 1.965e9 / 1e12, "f64": 148 * 64 * 2 * 1.965e9 / 1e12}
-# dram__bytes_read.sum + dram__bytes_write.sum of one gray_integrate launch in the committed `ncu --set full`
-# capture (profiles/r01_README.md: 260.2 MB for 2^22 photons, fp32), per photon; the launch of this run is
-# scaled from it (a capture at 2^28 photons would replay a 3.7 s kernel ~40 times)
-NCU_DRAM_BYTES_PER_PHOTON = 62.04
+# dram__bytes_read.sum + dram__bytes_write.sum of one gray_integrate launch of the default workload (2^30 photons,
+# fp32) from the committed ncu capture profiles/r01_integrate_f2_dram_2p30.csv: 40.217 GB + 39.874 GB, per photon
+NCU_DRAM_BYTES_PER_PHOTON = 74.59
 
 
 def parse():
@@ -303,7 +302,7 @@ def run_gray(args):
                "integrator_mix": g.gray_packed_peak(2) / lane_peak}
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                 "traffic": (NCU_DRAM_BYTES_PER_PHOTON * n) if (NCU_DRAM_BYTES_PER_PHOTON and args.prec == "f32") else None,
-                "traffic_source": "ncu dram bytes per photon at 2^22 photons x photons of this launch",
+                "traffic_source": "ncu dram bytes per photon of the 2^30-photon launch (profiles/) x photons of this launch",
                 "kernel": "gray::integrate_kernel", "kernel_ms": kern_ms, "kernel_share_of_step": kern_ms * args.steps / ms,
                 "flops_per_photon_step": flops, "flops_source": "oracle operation tally (add=sub=mul=div=sqrt=sin=cos=1)",
                 "peak_source": "148 SMs x %d lanes x 2 x 1.965 GHz (DESIGN.md)" % (128 if args.prec == "f32" else 64),
