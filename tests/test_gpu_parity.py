@@ -177,6 +177,15 @@ def test_schedules_intervals_and_resume_are_bit_identical():
                 base = cur
             else:
                 assert all(torch.equal(u.view(torch.uint8), v.view(torch.uint8)) for u, v in zip(base, cur)), kw
+        # the xi-monitor kernels (paper P:103-107) are a separate instantiation: same check, on rays that use the fallback
+        outs_xi = []
+        for kw in (dict(), dict(schedule=g.SCHED_STATIC, photons_per_thread=1)):
+            b = g.PhotonBatch(nx * ny, prec)
+            g.gray_init_rays(b, 0.99, wl.R_OBS, 5.0, W, nx, ny)
+            g.gray_integrate(b, max_steps=wl.MAX_STEPS, params=g.StepParams(rule=g.STEP_EQ2, xi_epsilon=1e-3, **kw))
+            outs_xi.append((b.x.clone(), b.k.clone(), b.status.clone(), b.steps.clone(), g.gray_integrate_counters(b)["fallback_steps"]))
+        assert outs_xi[0][4] == outs_xi[1][4] > 0
+        assert all(torch.equal(u.view(torch.uint8), v.view(torch.uint8)) for u, v in zip(outs_xi[0][:4], outs_xi[1][:4]))
         # resume: 100 steps, then 250 more, then to the end == one uninterrupted call
         b = g.PhotonBatch(nx * ny, prec)
         g.gray_init_rays(b, a, wl.R_OBS, inc, W, nx, ny)
