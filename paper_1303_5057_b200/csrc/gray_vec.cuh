@@ -56,7 +56,7 @@ GRAY_DEV void vpack(f2& v, const float s[2]) { v = f2_pack(s[0], s[1]); }
 
 // ---- add, sub, mul, fma: one rounding each -----------------------------------------------------------
 GRAY_DEV float vadd(float a, float b) { return __fadd_rn(a, b); }
-GRAY_DEV float vsub(float a, float b) {      // explicit sub.rn: __fsub_rn was seen contracted with a feeding __fmul_rn
+GRAY_DEV float vsub(float a, float b) {      // sub.rn spelled out: the same instruction form as the packed build's
   float d;
   asm("sub.rn.f32 %0, %1, %2;" : "=f"(d) : "f"(a), "f"(b));
   return d;
