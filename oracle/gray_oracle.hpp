@@ -36,7 +36,8 @@
 //   shadow statistics     : Bardeen closed-form curve (area, alpha extent, D,
 //                           <R>, A), an exact synthetic disc, paper eqs. 11-14
 // Parity unpinned (GPU-vs-oracle only): the final state of CAPTURED rays at
-// 1.01 r_h, the EQ2 step rule's min() selection on individual steps, and the
+// 1.01 r_h for a != 0 (a = 0: phi by the orbit integral, k^r by the null condition),
+// the EQ2 step rule's min() selection on individual steps, and the
 // Kerr (a != 0) equatorial crossing radius beyond the invariants above.
 #pragma once
 #include <cmath>

@@ -405,3 +405,23 @@ def test_reduced_system_integration_classifies_conserves_and_converges_to_the_fu
         dist.append(np.max(np.abs(yr[1:4] - yf[1:4])))
     assert 10 < dq[0] / dq[1] < 40 and 10 < dq[1] / dq[2] < 40, dq                 # 4th order or better
     assert 10 < dist[0] / dist[1] < 40 and 10 < dist[1] / dist[2] < 40, dist
+
+
+def test_captured_rays_final_state_schwarzschild_orbit_integral():
+    # The final state of CAPTURED rays (stopped at r < 1.01 r_h) pinned for a = 0: an equatorial ray (i = 90 deg,
+    # beta = 0) with impact parameter b < sqrt(27) has no turning point, and phi swept from the start to the final
+    # radius is the textbook integral  int_{u0}^{uf} du / sqrt(1/b^2 - u^2 (1 - 2u)),  u = 1/r.
+    from scipy import integrate as sint
+    a = 0.0
+    for al in (1.0, 3.0, 4.5, 5.1):
+        y0 = o.init_ray(a, 1000.0, 90.0, al, 0.0)
+        y, st, n = o.integrate(a, y0, 1 / 32, 1.01 * 2.0, 1010.0, o.STEP_EQ2, 20000)
+        assert st == o.CAPTURED and 2.0 < y[1] < 2.02 and abs(y[2] - np.pi / 2) < 1e-12
+        E, L, Q, _ = o.invariants(a, y0)
+        b = abs(L) / E
+        f = lambda u: 1.0 / (b * b) - u * u * (1.0 - 2.0 * u)
+        exact = sint.quad(lambda u: 1.0 / np.sqrt(f(u)), 1.0 / y0[1], 1.0 / y[1], epsabs=1e-13, epsrel=1e-13, limit=400)[0]
+        assert abs(abs(y[3] - y0[3]) - exact) < 2e-5 * exact, (al, abs(y[3] - y0[3]), exact)
+        # and the radial momentum there follows from the null condition with the conserved E, L
+        kr_exact = np.sqrt(E * E - (1 - 2 / y[1]) * L * L / y[1] ** 2)   # > 0: r grows with lambda, the ray is traced backwards
+        assert abs(y[5] - kr_exact) < 2e-2 * kr_exact               # the last steps next to the coordinate singularity: ~1 %
