@@ -64,7 +64,12 @@ def bardeen_curve(a, inc_deg, n=200001):
 
 
 def bardeen_rho(a, inc_deg, vartheta):
-    """Radius of the critical curve along the spoke at polar angle vartheta about the image origin."""
+    """Radius of the critical curve along the spoke at polar angle vartheta about the image origin.
+    Symmetries: i -> 180 - i leaves the curve unchanged (it depends on sin i and cos^2 i); a -> -a mirrors alpha."""
+    if inc_deg > 90.0:
+        inc_deg = 180.0 - inc_deg
+    if a < 0.0:
+        return bardeen_rho(-a, inc_deg, np.pi - np.asarray(vartheta, dtype=float))
     al, be = bardeen_curve(a, inc_deg)
     ang = np.arctan2(be, al)          # pi ... 0, decreasing along the curve
     rho = np.hypot(al, be)

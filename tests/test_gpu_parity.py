@@ -75,6 +75,7 @@ def _run_gpu_from_oracle_init(a, inc, W, nx, ny, prec, rule, **kw):
     (0.0, 60.0, 10.0, 64, 64, g.STEP_REL),        # C1 with the configs' literal rule
     (0.9, 60.0, 10.0, 61, 45, g.STEP_EQ2),        # C2 geometry, ragged size (2745 = 21 blocks + 57)
     (0.99, 90.0, 12.0, 48, 48, g.STEP_EQ2),       # C3 geometry
+    (-0.8, 120.0, 10.0, 48, 40, g.STEP_EQ2),      # retrograde spin, observer below the equator (theta starts mirrored)
 ])
 def test_integrate_f64_matches_oracle(a, inc, W, nx, ny, rule):
     # north_star: "fp64 GPU vs oracle: <= 1e-9 relative"
@@ -117,7 +118,8 @@ def test_integrate_f64_matches_oracle(a, inc, W, nx, ny, rule):
 
 
 @pytest.mark.parametrize("a,inc,W,nx,ny", [(0.0, 60.0, 10.0, 64, 64), (0.9, 60.0, 10.0, 64, 64), (0.99, 90.0, 12.0, 64, 64),
-                                           (0.7, 45.0, 15.0, 64, 64)])
+                                           (0.7, 45.0, 15.0, 64, 64),
+                                           (-0.8, 120.0, 10.0, 64, 64)])     # retrograde spin, observer below the equator
 def test_integrate_f32_matches_fp64_oracle(a, inc, W, nx, ny):
     # north_star tolerances for fp32 GPU vs fp64 oracle, protocol of DESIGN.md reading R11
     b = g.PhotonBatch(nx * ny, g.GRAY_F32)
