@@ -193,7 +193,7 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
             for (int l = 0; l < N; ++l) c_fallback += (rej[l] && have[l]) ? 1u : 0u;
           }
           const V z = RED ? vfma(K.zero, y[6], vmul(K.zero, y[5])) : nonfinite_probe(K, y);
-          const V r = vadd(y[1], K.rp);
+          const V r = y[1];                       // the tests compare heights above the horizon (Consts::r_cap, r_esc)
           // Bookkeeping.  Common case first, with one branch for the whole thread: every slot's theta still in
           // [0, pi/2] (no eq. (3) remap, no fold) and no slot finished.
           S th[N], rr[N], zz[N];
@@ -255,7 +255,7 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
           bool rej[N];
           rk4_step<false>(K, w, wc, dl, rej);
           const V z = nonfinite_probe(K, w);
-          const V r = vadd(w[1], K.rp);
+          const V r = w[1];
           S th[N], ph[N], kh[N], c2[N], c6[N];
           int wm[N];
           bool adv[N];

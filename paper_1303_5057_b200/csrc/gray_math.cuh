@@ -48,7 +48,7 @@ struct Consts {
   V zero, one, mone, two, m2, half, nhalf, sixth, ninth;
   // sin / cos (float builds): quadrant reduction and minimax polynomials, see sincos_v
   V two_over_pi, magic, npio2_hi, npio2_lo, s1, s2, s3, c1, c2, c3, c4;
-  S r_cap, r_esc;                         // termination radii
+  S r_cap, r_esc;                         // termination radii, as heights above the horizon (r - r_+): the kernel's radial variable
   S xi_eps;                               // epsilon of the xi monitor (paper eq. 4); 0 = off
 };
 
@@ -68,7 +68,7 @@ __host__ inline Consts<V> make_consts(double a, double h, double r_cap, double r
   K.npio2_hi = B(-1.57079637050628662109375); K.npio2_lo = B(4.371139000186241e-08);
   K.s1 = B(-1.666666418e-01); K.s2 = B(8.332700469e-03); K.s3 = B(-1.957778732e-04);
   K.c1 = B(-0.5); K.c2 = B(4.166664928e-02); K.c3 = B(-1.388748409e-03); K.c4 = B(2.445036807e-05);
-  K.r_cap = (S)r_cap; K.r_esc = (S)r_esc;
+  K.r_cap = (S)(r_cap - (1.0 + root)); K.r_esc = (S)(r_esc - (1.0 + root));   // differences formed in double
   return K;
 }
 
@@ -497,7 +497,7 @@ GRAY_DEV V nonfinite_probe(const Consts<V>& K, const V y[8]) {
 
 // status of one photon after a full step: BAD(3) / CAPTURED(1) / ESCAPED(2) / LIVE(0), in that order
 template <typename S>
-GRAY_DEV int state_status(S z, S r, S r_cap, S r_esc) {
+GRAY_DEV int state_status(S z, S r, S r_cap, S r_esc) {     // r, r_cap, r_esc: heights above the horizon
   if (!(z == S(0))) return 3;
   if (r < r_cap) return 1;
   if (r > r_esc) return 2;

@@ -320,3 +320,34 @@ def test_integrate_host_matches_device_path():
         assert torch.equal(k_out.view(torch.uint8), b.k.cpu().view(torch.uint8))
         assert torch.equal(status, b.status.cpu()) and torch.equal(steps, b.steps.cpu())
         assert cnt["photon_steps"] == cnt_dev["photon_steps"] and cnt["photons_done"] == n
+
+
+@pytest.mark.parametrize("prec", [g.GRAY_F32, g.GRAY_F64])
+def test_paper_horizon_standoff_delta(prec):
+    # the paper's own termination: stop at r_bh + delta with delta ~ 1e-6 (r_capture_factor = 0); only eq. (2)'s
+    # (r - r_bh) / (2 |dr/dlambda|) limiter lets a ray get there.  The kernel compares heights above the horizon, so the
+    # threshold 1e-6 is exact in fp32 too.
+    a, inc, W, nx, ny = 0.9, 60.0, 10.0, 48, 48
+    f32 = prec == g.GRAY_F32
+    delta = float(gold_delta())
+    b = g.PhotonBatch(nx * ny, prec)
+    g.gray_init_rays(b, a, wl.R_OBS, inc, W, nx, ny)
+    g.gray_integrate(b, max_steps=wl.MAX_STEPS, params=g.StepParams(rule=g.STEP_EQ2, r_capture_factor=0.0, horizon_delta=delta))
+    y, st, n = gpu_state(b)
+    ref = o.trace(a, wl.R_OBS, inc, W, nx, ny, rule=o.STEP_EQ2, cap_factor=0.0, horizon_delta=delta, init_f32=f32, threads=8)
+    al, be = grid_pixels(W, nx, ny)
+    band = edge_band(a, inc, al, be)
+    assert np.all((st == ref["status"]) | band) and not np.any(st == g.LIVE)
+    cap = (st == g.CAPTURED) & (ref["status"] == o.CAPTURED) & ~band
+    assert cap.sum() > 100
+    rh = o.horizon(a)
+    # every captured ray ends within delta of the horizon, having taken ~ log2(0.01 / delta) more steps than to 1.01 r_h
+    assert np.all(y[cap, 1] - rh < 2 * delta) and np.all(y[cap, 1] - rh > (0.0 if f32 else 0.2 * delta))
+    assert np.all(np.abs(n[cap] - ref["steps"][cap]) <= (3 if f32 else 1))
+    xi, eta = xi_eta_of(a, ref["y0"])
+    assert np.all(((st == g.CAPTURED) == exact_capture(a, xi, eta)) | band)
+
+
+def gold_delta():
+    import golden_values
+    return golden_values.load()["horizon_standoff"]
