@@ -397,3 +397,23 @@ def test_reduced_system_matches_oracle(prec, a, inc, W):
     tol = 5e-6 if f32 else 1e-12            # fp32: the rounding of the stored state, not drift
     assert np.max(np.abs(inv1[esc, 0] - inv0[esc, 0])) <= tol
     assert np.max(np.abs(inv1[esc, 1] - inv0[esc, 1]) / np.maximum(np.abs(inv0[esc, 1]), 1.0)) <= tol
+
+
+def test_equatorial_projection_with_xi_monitor_matches_oracle():
+    # the two options together (the paper's production scheme projecting a face-on grid): fp64, so that
+    # the comparison is not blurred by precision - every face-on ray runs over the pole (reading R20)
+    a, inc, nx, ny, W = 0.95, 0.0, 64, 48, 10.0
+    b = g.PhotonBatch(nx * ny, g.GRAY_F64)
+    g.gray_init_rays(b, a, wl.R_OBS, inc, W, nx, ny)
+    g.gray_integrate(b, max_steps=wl.MAX_STEPS, params=g.StepParams(rule=g.STEP_EQ2, stop_at_equator=True, xi_epsilon=1e-3))
+    fb = g.gray_integrate_counters(b)["fallback_steps"]
+    torch.cuda.synchronize()
+    y = torch.cat([b.x, b.k], dim=1).cpu().numpy()
+    st = b.status.cpu().numpy().astype(np.int32)
+    ns = b.steps.cpu().numpy().astype(np.int64)
+    ref = o.trace(a, wl.R_OBS, inc, W, nx, ny, rule=o.STEP_EQ2, threads=16, stop_at_equator=True, xi_eps=1e-3)
+    assert fb > 0 and np.mean(st == ref["status"]) >= 0.995
+    same = (st == ref["status"]) & (ns == ref["steps"]) & (st == g.EQUATOR)
+    assert same.mean() > 0.7
+    err = np.abs(y[same][:, [1, 3]] - ref["y"][same][:, [1, 3]]) / np.maximum(1.0, np.abs(ref["y"][same][:, [1, 3]]))
+    assert np.quantile(err, 0.99) <= 1e-7, np.quantile(err, 0.99)
