@@ -36,7 +36,8 @@
 //   shadow statistics     : Bardeen closed-form curve (area, alpha extent, D,
 //                           <R>, A), an exact synthetic disc, paper eqs. 11-14
 // Parity unpinned (GPU-vs-oracle only): the final state of CAPTURED rays at
-// 1.01 r_h for a != 0 (a = 0: phi by the orbit integral, k^r by the null condition),
+// 1.01 r_h off the equatorial plane for a != 0 (a = 0: phi by the orbit integral, k^r by
+// the null condition; Kerr equatorial rays: phi, k^r by the Bardeen 1972 quadrature),
 // the EQ2 step rule's min() selection on individual steps, and the
 // Kerr (a != 0) equatorial crossing radius beyond the invariants above.
 #pragma once

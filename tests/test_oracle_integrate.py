@@ -425,3 +425,30 @@ def test_captured_rays_final_state_schwarzschild_orbit_integral():
         # and the radial momentum there follows from the null condition with the conserved E, L
         kr_exact = np.sqrt(E * E - (1 - 2 / y[1]) * L * L / y[1] ** 2)   # > 0: r grows with lambda, the ray is traced backwards
         assert abs(y[5] - kr_exact) < 2e-2 * kr_exact               # the last steps next to the coordinate singularity: ~1 %
+
+
+def test_equatorial_kerr_rays_against_the_bardeen_1972_quadrature():
+    # Kerr pin for whole trajectories, captured ones included: a ray in the equatorial plane (i = 90 deg, beta = 0)
+    # stays there, and with E = -k_t, L = k_phi (textbook, Bardeen, Press & Teukolsky 1972)
+    #     dphi/dl = [(1 - 2/r) L + (2a/r) E] / Delta,      (dr/dl)^2 = E^2 + (a^2 E^2 - L^2)/r^2 + 2 (L - a E)^2 / r^3,
+    # so phi along a ray without a turning point is a quadrature in r.  Checked for rays captured on the prograde and on
+    # the retrograde side (frame dragging reverses dphi/dl of the latter near the horizon).
+    from scipy import integrate as sint
+    a = 0.9
+    rh = o.horizon(a)
+    checked = 0
+    for al in (-2.5, -1.0, 1.0, 3.0, 5.5):
+        y0 = o.init_ray(a, 1000.0, 90.0, al, 0.0)
+        y, st, n = o.integrate(a, y0, 1 / 32, 1.01 * rh, 1010.0, o.STEP_EQ2, 20000)
+        assert abs(y[2] - np.pi / 2) < 1e-12
+        if st != o.CAPTURED:
+            continue
+        E, L, Q, _ = o.invariants(a, y0)
+        dphi = lambda r: ((1 - 2 / r) * L + 2 * a * E / r) / (r * r - 2 * r + a * a)
+        rdot = lambda r: np.sqrt(E * E + (a * a * E * E - L * L) / r ** 2 + 2 * (L - a * E) ** 2 / r ** 3)
+        sweep = sint.quad(lambda r: dphi(r) / rdot(r), y[1], y0[1], epsabs=1e-13, epsrel=1e-13, limit=800)[0]
+        got = y0[3] - y[3]                      # the physical photon runs from the hole (y) out to the observer (y0)
+        assert abs(got - sweep) < 5e-5 * max(1.0, abs(sweep)), (al, got, sweep)
+        assert abs(y[5] - rdot(y[1])) < 2e-2 * rdot(y[1])
+        checked += 1
+    assert checked >= 4
