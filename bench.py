@@ -46,7 +46,9 @@ def parse():
                     "the north star's 2^30; lowered, and said so in config.workload, if the device lacks the 40 GB it needs)")
     ap.add_argument("--prec", default="f32", choices=["f32", "f64"])
     ap.add_argument("--rule", default="eq2", choices=["eq2", "rel"])
-    ap.add_argument("--case", default="realistic", choices=["realistic", "peak"])
+    ap.add_argument("--case", default="realistic", choices=["realistic", "peak", "projection"],
+                    help="projection = the paper's first benchmark (P:130-140, Fig. 4): run time of the grid projection "
+                         "onto the equatorial plane (a = 0.95, i = 60 deg) against the number of rays")
     ap.add_argument("--schedule", default="refill", choices=["refill", "static"])
     ap.add_argument("--refill-interval", type=int, default=0)
     ap.add_argument("--photons-per-thread", type=int, default=0, help="0 = library default (2 for f32: packed FFMA2), 1, 2")
@@ -342,8 +344,49 @@ def run_gray(args):
         dist.destroy_process_group()
 
 
+def run_projection(args):
+    """Paper's Fig. 4: run time of the equatorial-plane grid projection, a = 0.95, i = 60 deg, against
+    the number of rays n (square grids over +-10 M).  Host wall clock around init -> integrate -> counters (what a
+    user waits for), best of 5; the paper finds a launch floor of ~20 ms and linear growth beyond ~1e4 rays on its
+    Tesla M2090 in double precision."""
+    import torch
+
+    import paper_1303_5057_b200 as g
+    from paper_1303_5057_b200 import workloads as wl
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    rows = []
+    for prec_name, prec in (("f64", g.GRAY_F64), ("f32", g.GRAY_F32)):
+        for log2n in range(8, 27, 2):
+            side = 2 ** (log2n // 2)
+            b = g.PhotonBatch(side * side, prec)
+            params = g.StepParams(rule=g.STEP_EQ2, stop_at_equator=True)
+            best, steps = 1e30, 0
+            for rep in range(6):
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                g.gray_init_rays(b, 0.95, wl.R_OBS, 60.0, 10.0, side, side)
+                g.gray_integrate(b, max_steps=wl.MAX_STEPS, params=params)
+                steps = g.gray_integrate_counters(b)["photon_steps"]          # synchronises
+                dt = time.perf_counter() - t0
+                if rep:
+                    best = min(best, dt)
+            rows.append({"precision": prec_name, "rays": side * side, "ms": 1e3 * best, "photon_steps": steps,
+                         "ns_per_photon_step": 1e9 * best / max(1, steps)})
+    out = {"metric": "run time of the equatorial-plane grid projection vs number of rays", "unit": "ms", "n_gpus": 1,
+           "data": "synthetic", "higher_is_better": False,
+           "config": {"workload": "paper Fig. 4: a=0.95, i=60 deg, square grids over +-10 M at r_obs=1000 M, eq. (2) rule, "
+                                  "stop at the equatorial plane", "timer": "host wall clock, best of 5"},
+           "rows": rows, "paper_context": "Tesla M2090, double precision: ~20 ms floor below ~1e4 rays, then linear (P:136-138)"}
+    print(json.dumps(out), flush=True)
+
+
 def main():
     args = parse()
+    if args.case == "projection" and args.impl != "reference":
+        run_projection(args)
+        return
     if args.impl == "reference":
         run_reference(args)
     else:
