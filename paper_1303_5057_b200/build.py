@@ -3,6 +3,8 @@
     python -m paper_1303_5057_b200.build [--force] [--verbose]
 
 Plain nvcc, in-tree output (the .so travels with the repository snapshot to the GPU box).
+GRAY_NVCC_EXTRA (environment) appends flags, e.g. "-DGRAY_BLOCK=64 -DGRAY_F2_MIN_BLOCKS=8" or "-DGRAY_COMP_MASK=0x6e":
+the tuning macros of csrc/gray_integrate.cu and csrc/gray_math.cuh (DESIGN.md lists what they measured).
 """
 import os
 import subprocess
