@@ -56,6 +56,9 @@ def parse():
     ap.add_argument("--xi-eps", type=float, default=0.0, help="epsilon of the paper's xi monitor (P:107); 0 = off")
     ap.add_argument("--e2e-log2n", type=int, default=-1, help="photons per GPU of the host-buffer run (default min(log2n, 26))")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--dist-backend", default="nccl", help="torch.distributed backend of the N > 1 run (the data path has no "
+                    "collective; only the timing / counter reduction uses it)")
+    ap.add_argument("--share-gpu", action="store_true", help="testing only: all ranks on cuda:0 (use with --dist-backend gloo)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--ref-log2n", type=int, default=18, help="--impl reference: photons of the strided sample per step")
     return ap.parse_args()
@@ -172,9 +175,14 @@ def run_gray(args):
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (libgray has no CPU path)")
+    if args.share_gpu:
+        local = 0
     torch.cuda.set_device(local)
     if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        if args.dist_backend == "nccl":
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        else:
+            dist.init_process_group(args.dist_backend)
     dev = torch.device("cuda", local)
 
     c4 = wl.C4
