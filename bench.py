@@ -34,6 +34,10 @@ PEAK_TFLOPS = {"f32": 148 * 128 * 2 * 1.965e9 / 1e12, "f64": 148 * 64 * 2 * 1.96
 # dram__bytes_read.sum + dram__bytes_write.sum of one gray_integrate launch of the default workload (2^30 photons,
 # fp32) from the committed ncu capture profiles/r01_integrate_f2_dram_2p30.csv: 40.217 GB + 39.874 GB, per photon
 NCU_DRAM_BYTES_PER_PHOTON = 74.59
+# FP32 operations the packed kernel EXECUTES per photon-step (FMA = 2), from the instruction counts of the committed
+# ncu capture (profiles/r01_README.md: FFMA2 166.4, FMUL2 179.4, FADD2 51.1 per warp per step of its 64 photons, plus
+# scalar FADD): fewer than the oracle's tally because the kernel contracts the Christoffel sums analytically
+NCU_EXECUTED_FLOPS_PER_PHOTON_STEP = 563
 
 
 def parse():
@@ -314,6 +318,7 @@ def run_gray(args):
                 "traffic": (NCU_DRAM_BYTES_PER_PHOTON * n) if (NCU_DRAM_BYTES_PER_PHOTON and args.prec == "f32") else None,
                 "traffic_source": "ncu dram bytes per photon of the 2^30-photon launch (profiles/) x photons of this launch",
                 "kernel": "gray::integrate_kernel", "kernel_ms": kern_ms, "kernel_share_of_step": kern_ms * args.steps / ms,
+                "executed_flops_per_photon_step": NCU_EXECUTED_FLOPS_PER_PHOTON_STEP if (args.prec == "f32" and args.photons_per_thread != 1 and args.system == "full" and args.xi_eps == 0) else None,
                 "flops_per_photon_step": flops, "flops_source": "oracle operation tally (add=sub=mul=div=sqrt=sin=cos=1)",
                 "peak_source": "148 SMs x %d lanes x 2 x 1.965 GHz (DESIGN.md)" % (128 if args.prec == "f32" else 64),
                 "fma_microbench_tflops": fma_peak, "frac_of_fma_microbench": achieved / fma_peak,
