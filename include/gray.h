@@ -69,6 +69,7 @@ typedef enum { GRAY_SYS_FULL = 0, GRAY_SYS_REDUCED = 1 } gray_system;
 
 typedef enum { GRAY_LIVE = 0, GRAY_CAPTURED = 1, GRAY_ESCAPED = 2, GRAY_BAD = 3,
                GRAY_EQUATOR = 4 /* reached theta = pi/2 (stop_at_equator only) */ } gray_ray_status;
+#define GRAY_N_STATUS 5   /* number of gray_ray_status values = length of gray_classify's counts_host */
 
 /* How photons are mapped to threads by gray_integrate.
  *   GRAY_SCHED_REFILL  persistent warps; a lane whose photon has terminated fetches the next live
@@ -150,7 +151,8 @@ typedef struct {
                                 by two Newton iterations - ordinary, counted steps of size
                                 dlambda = -(theta - pi/2) / k^theta - and gets status GRAY_EQUATOR; the stored
                                 state is the one after the second (theta within rounding of pi/2).  Test
-                                order: BAD, CAPTURED, EQUATOR, ESCAPED.  gray_classify counts statuses 0-3 only.
+                                order: BAD, CAPTURED, EQUATOR, ESCAPED.  The landing steps are taken even when they pass
+                                max_steps (by at most 2), as the crossing step itself decides the status.
                                 Not available together with `frozen`.                                 */
   double xi_epsilon;         /* > 0: the paper's production pole treatment: after every RK4 step
                                 xi of eq. (4) is evaluated at the new state; if |xi + 1| > xi_epsilon (the
@@ -190,8 +192,10 @@ typedef struct {
 GRAY_API int gray_integrate_counters(const void* workspace_dev, gray_counters* counters_host, void* cuda_stream);
 
 /* Per-pixel capture flags (capture_map[p] = 1 iff status[p] == GRAY_CAPTURED, else 0; may be NULL)
- * and the number of photons in each gray_ray_status (counts_host[4]).  Synchronises the stream.     */
-GRAY_API int gray_classify(const gray_state* state, uint8_t* capture_map_dev, uint64_t counts_host[4],
+ * and the number of photons in each gray_ray_status: counts_host[s], s = GRAY_LIVE .. GRAY_EQUATOR
+ * (GRAY_N_STATUS = 5 entries; a status byte outside that range is counted nowhere, so the counts sum
+ * to n exactly when every byte is a valid status).  Synchronises the stream.                        */
+GRAY_API int gray_classify(const gray_state* state, uint8_t* capture_map_dev, uint64_t counts_host[GRAY_N_STATUS],
                   void* workspace_dev, size_t workspace_bytes, void* cuda_stream);
 
 /* Shadow / photon-ring statistics of a grid image (reading R13):

@@ -24,8 +24,11 @@
 //                           classifier (Kerr), Schwarzschild deflection
 //                           quadrature, reflection / spin-flip symmetries,
 //                           the face-on critical radius next to P:91's value
-//   pole treatment        : advance() with xi_eps > 0 (paper P:103-107) against the
-//                           exact classifier on rays next to the spin axis
+//   pole treatment        : advance() with xi_eps > 0 (paper P:103-107): ONE step against
+//                           y_old + (dl/9) rhs(y_old) / the RK4 result formed in numpy from
+//                           the pinned rhs, step_size, metric (branch by xi from the metric;
+//                           the 9 from the paper's text); whole rays next to the spin axis
+//                           against the exact classifier
 //   equatorial projection : a = 0 line of nodes and orbit integral (phi, r at the
 //                           crossing to 2e-6); Kerr: invariants at the landed state,
 //                           reflection symmetry

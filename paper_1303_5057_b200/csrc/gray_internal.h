@@ -19,10 +19,10 @@ struct Workspace {
   unsigned long long photons_live;
   unsigned long long fallback_steps;
   unsigned long long pad1[11];
-  unsigned long long counts[4];           // gray_classify: photons per status
+  unsigned long long counts[GRAY_N_STATUS];  // gray_classify: photons per status
   unsigned long long sum_col, sum_row;    // gray_shadow_edge: sums of captured pixel indices
   unsigned int min_col, max_col;          //                   extreme captured columns
-  unsigned long long pad2[9];
+  unsigned long long pad2[8];
   double stats[8];                        // gray_shadow_edge: the doubles of gray_shadow_stats
   unsigned long long n_captured;
   unsigned long long pad3[7];

@@ -6,11 +6,14 @@ namespace gray {
 
 __device__ __forceinline__ unsigned int warp_sum_u32(unsigned int v) { return __reduce_add_sync(0xffffffffu, v); }
 
-// status -> capture flags + histogram of the four statuses.  16 photons per thread per iteration when
-// the buffers allow 16-byte accesses.
+// status -> capture flags + histogram of the GRAY_N_STATUS statuses (bytes outside 0 .. GRAY_N_STATUS-1 are counted
+// nowhere).  16 photons per thread per iteration when the buffers allow 16-byte accesses; the bytes of a word are
+// compared four at a time (__vcmpeq4).
 __global__ void __launch_bounds__(256) classify_kernel(const uint8_t* __restrict__ status, uint8_t* __restrict__ cmap,
                                                        unsigned long long n, int vec_ok, Workspace* ws) {
-  unsigned int c[4] = {0, 0, 0, 0};
+  unsigned int c[GRAY_N_STATUS];
+#pragma unroll
+  for (int q = 0; q < GRAY_N_STATUS; ++q) c[q] = 0;
   const unsigned long long tid = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
   const unsigned long long nthreads = (unsigned long long)gridDim.x * blockDim.x;
   const unsigned long long nvec = vec_ok ? n / 16 : 0;
@@ -20,24 +23,20 @@ __global__ void __launch_bounds__(256) classify_kernel(const uint8_t* __restrict
     unsigned int out[4];
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
-      unsigned int o = 0;
 #pragma unroll
-      for (int b = 0; b < 4; ++b) {
-        const unsigned int s = (in[q] >> (8 * b)) & 0xffu;
-        c[s & 3u] += 1u;
-        o |= (s == GRAY_CAPTURED ? 1u : 0u) << (8 * b);
-      }
-      out[q] = o;
+      for (int s = 0; s < GRAY_N_STATUS; ++s) c[s] += __popc(__vcmpeq4(in[q], 0x01010101u * (unsigned int)s)) >> 3;
+      out[q] = __vcmpeq4(in[q], 0x01010101u * (unsigned int)GRAY_CAPTURED) & 0x01010101u;
     }
     if (cmap) ((uint4*)cmap)[v] = make_uint4(out[0], out[1], out[2], out[3]);
   }
   for (unsigned long long p = nvec * 16 + tid; p < n; p += nthreads) {
     const unsigned int s = status[p];
-    c[s & 3u] += 1u;
+#pragma unroll
+    for (int q = 0; q < GRAY_N_STATUS; ++q) c[q] += (s == (unsigned int)q) ? 1u : 0u;
     if (cmap) cmap[p] = (s == GRAY_CAPTURED) ? 1 : 0;
   }
 #pragma unroll
-  for (int q = 0; q < 4; ++q) {
+  for (int q = 0; q < GRAY_N_STATUS; ++q) {
     const unsigned int t = warp_sum_u32(c[q]);
     if ((threadIdx.x & 31) == 0 && t) atomicAdd(&ws->counts[q], (unsigned long long)t);
   }
@@ -218,7 +217,7 @@ static unsigned int reduce_grid(unsigned long long n, unsigned long long per_thr
 
 extern "C" {
 
-int gray_classify(const gray_state* state, uint8_t* capture_map_dev, uint64_t counts_host[4], void* workspace_dev,
+int gray_classify(const gray_state* state, uint8_t* capture_map_dev, uint64_t counts_host[GRAY_N_STATUS], void* workspace_dev,
                   size_t workspace_bytes, void* cuda_stream) {
   using namespace gray;
   int rc = check_state(state, false);
@@ -234,10 +233,10 @@ int gray_classify(const gray_state* state, uint8_t* capture_map_dev, uint64_t co
     classify_kernel<<<reduce_grid(state->n, 16), 256, 0, stream>>>(state->status_dev, capture_map_dev, state->n, vec_ok, ws);
     GRAY_CUDA(cudaGetLastError());
   }
-  unsigned long long c[4];
+  unsigned long long c[GRAY_N_STATUS];
   GRAY_CUDA(cudaMemcpyAsync(c, &ws->counts[0], sizeof c, cudaMemcpyDeviceToHost, stream));
   GRAY_CUDA(cudaStreamSynchronize(stream));
-  for (int q = 0; q < 4; ++q) counts_host[q] = c[q];
+  for (int q = 0; q < GRAY_N_STATUS; ++q) counts_host[q] = c[q];
   return GRAY_OK;
 }
 

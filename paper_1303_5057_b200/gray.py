@@ -12,6 +12,7 @@ GRAY_F32, GRAY_F64 = 0, 1
 STEP_REL, STEP_EQ2 = 0, 1
 SYS_FULL, SYS_REDUCED = 0, 1
 LIVE, CAPTURED, ESCAPED, BAD, EQUATOR = 0, 1, 2, 3, 4
+N_STATUS = 5
 SCHED_REFILL, SCHED_STATIC = 0, 1
 PIXELS_GRID, PIXELS_RANDOM, PIXELS_POLAR = 0, 1, 2
 
@@ -180,8 +181,8 @@ def gray_integrate_counters(batch):
 
 
 def gray_classify(batch, capture_map=None):
-    """Returns counts[4] (LIVE, CAPTURED, ESCAPED, BAD); fills capture_map (uint8 tensor of n) if given."""
-    counts = (C.c_uint64 * 4)()
+    """Returns counts[5] (LIVE, CAPTURED, ESCAPED, BAD, EQUATOR); fills capture_map (uint8 tensor of n) if given."""
+    counts = (C.c_uint64 * N_STATUS)()
     _check(lib().gray_classify(C.byref(batch.c), _ptr(capture_map), counts, _ptr(batch.workspace),
                                batch.workspace.numel(), _stream()))
     return [int(v) for v in counts]

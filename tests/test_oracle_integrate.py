@@ -244,6 +244,50 @@ def test_pole_treatment_xi_monitor_cures_the_pole_failures():
     assert esc.any() and np.array_equal(p2["y"][esc], c2["y"][esc]) and np.array_equal(p2["steps"][esc], c2["steps"][esc])
 
 
+def test_xi_monitor_fallback_is_one_euler_step_of_a_ninth_from_the_old_state():
+    # P:103-107 / reading R18, pinned step by step: after ONE step with xi_eps > 0 the state is
+    #   the RK4 result                              if |xi + 1| <= eps at the RK4 result,
+    #   y_old + (dlambda / 9) rhs(y_old)             otherwise
+    # (theta-remapped, one step counted either way), with xi + 1 formed here from the metric, the Euler step formed
+    # here in numpy from the separately pinned rhs / step_size, and 9 read from the paper's text (golden).
+    import xi_cases as xc
+    a, eps = xc.A_SPIN, xc.EPS
+    assert xc.NINE == 9.0
+    taken = {"rk4": 0, "euler": 0}
+    for y in xc.base_states():
+        for delta in (0.0, 1e-4, 3e-4, 4.5e-4, 5.5e-4, 8e-4, 2e-3, 1e-2, -4.5e-4, -5.5e-4, -5e-3):
+            z = xc.off_shell(y, delta)
+            rk, eu, xi1, dl = xc.expected_one_step(a, z)
+            if abs(abs(xi1) - eps) < 1e-9:
+                continue
+            got, status, steps = o.integrate(a, z, xc.H, 0.0, 1e9, o.STEP_EQ2, 1, xi_eps=eps)
+            assert steps == 1 and status == o.LIVE
+            want = eu if abs(xi1) > eps else rk
+            taken["euler" if abs(xi1) > eps else "rk4"] += 1
+            assert np.array_equal(got, want), (delta, xi1)
+            if abs(xi1) > eps:
+                # what a plausible misreading would give is far from rounding distance: Euler with dl/3, Euler with
+                # the NEW state's derivative, Euler from the new state, or keeping the RK4 step
+                scale = np.maximum(np.abs(want), 1.0)
+                alts = [z + (dl / 3.0) * o.rhs(a, z), z + (dl / 9.0) * o.rhs(a, rk), rk + (dl / 9.0) * o.rhs(a, rk), rk,
+                        z + dl * o.rhs(a, z)]
+                for alt in alts:
+                    assert np.max(np.abs(o.remap_theta(alt) - want) / scale) > 1e-6
+            # with the monitor off the RK4 step is kept whatever xi is
+            off, _, _ = o.integrate(a, z, xc.H, 0.0, 1e9, o.STEP_EQ2, 1, xi_eps=0.0)
+            assert np.array_equal(off, rk)
+    assert taken["rk4"] >= 15 and taken["euler"] >= 15, taken
+    # same under the configs' literal rule, and the fallback is not re-tested: a second step starts from the Euler state
+    z = xc.off_shell(xc.base_states()[0], 1e-2)
+    rk, eu, xi1, dl = xc.expected_one_step(a, z, rule=o.STEP_REL)
+    got, _, steps = o.integrate(a, z, xc.H, 0.0, 1e9, o.STEP_REL, 1, xi_eps=eps)
+    assert abs(xi1) > eps and np.array_equal(got, eu)
+    two, _, steps = o.integrate(a, z, xc.H, 0.0, 1e9, o.STEP_EQ2, 2, xi_eps=eps)
+    _, eu1, _, _ = xc.expected_one_step(a, z)
+    rk2, eu2, xi2, _ = xc.expected_one_step(a, eu1)
+    assert steps == 2 and np.array_equal(two, eu2 if abs(xi2) > eps else rk2)
+
+
 def test_equatorial_projection_schwarzschild_node_line_and_orbit_integral():
     # NEXT-2: follow rays to the equatorial plane.  Pins for a = 0, where the motion is planar:
     # (i) the plane of the orbit contains the origin, the observer direction o and the pixel offset, so its line of
