@@ -101,6 +101,10 @@ typedef struct {
   uint64_t seed;          /* random workload: key of the counter-based pixel generator               */
   uint64_t p0;            /* global index of photon 0 of this batch (sharding across GPUs / chunks)  */
   double r_lo;            /* polar workload: inner radius of the image-plane annulus (outer = half_width) */
+  void* resume_dev;       /* optional (may be NULL): n x 16 scalars of `prec`, 16-byte aligned, caller-owned.
+                             gray_integrate writes a record here for every photon it leaves GRAY_LIVE at
+                             max_steps and reads it back when a later call takes that photon up again; see
+                             gray_integrate.  Need not be initialised.                                   */
 } gray_state;
 
 /* Image plane -> initial photon states ("initial conditions ... as in Psaltis & Johannsen
@@ -174,6 +178,16 @@ GRAY_API size_t gray_workspace_bytes(uint64_t n);
  * order non-finite -> GRAY_BAD, r < r_capture -> GRAY_CAPTURED, r > r_escape -> GRAY_ESCAPED } until a
  * test fires or steps == max_steps (the photon then stays GRAY_LIVE and a later call resumes it).  The
  * stored state is the first one that satisfies a test.  x, k, status, steps are updated in place.
+ * Resuming (the paper's interactive mode takes "a few steps" per call, P:81 fn 5).  Inside the kernel a photon
+ * is carried in variables that the stored (t, r, theta, phi; k) do not hold exactly: the height above the horizon
+ * d = r - r_bh, the polar angle folded into [0, pi/2], and (GRAY_F32) the compensation terms of the state update.
+ *   state->resume_dev != NULL  these are saved for every photon left LIVE (64 B per photon in fp32, 128 B in fp64)
+ *                              and restored by the next call if the record still matches the stored r, theta and
+ *                              step count bit for bit (so a state edited by the caller is simply re-read): any
+ *                              sequence of calls then gives results BIT-IDENTICAL to one uninterrupted call.
+ *   state->resume_dev == NULL  each interruption rounds r and theta once and drops the compensation: results agree
+ *                              with the uninterrupted call to rounding error amplified along the ray (within the
+ *                              tolerances of the build, tests/test_gpu_parity.py), not bit for bit.
  * Asynchronous.  Counters of the call are left in the workspace for gray_integrate_counters().
  * Errors: GRAY_ERR_ARG, GRAY_ERR_DOMAIN, GRAY_ERR_WORKSPACE, GRAY_ERR_CUDA.                         */
 GRAY_API int gray_integrate(gray_state* state, uint64_t n_photons, uint32_t max_steps,

@@ -28,6 +28,7 @@ int check_state(const gray_state* st, bool need_image_fields) {
   if (!st->x_dev || !st->k_dev || !st->status_dev || !st->steps_dev) { set_error("state has a NULL device pointer"); return GRAY_ERR_ARG; }
   if (((uintptr_t)st->x_dev & 15) || ((uintptr_t)st->k_dev & 15)) { set_error("state.x_dev / k_dev must be 16-byte aligned"); return GRAY_ERR_ARG; }
   if ((uintptr_t)st->steps_dev & 3) { set_error("state.steps_dev must be 4-byte aligned"); return GRAY_ERR_ARG; }
+  if ((uintptr_t)st->resume_dev & 15) { set_error("state.resume_dev must be 16-byte aligned (or NULL)"); return GRAY_ERR_ARG; }
   if (need_image_fields) {
     if (!(st->a > -1.0 && st->a < 1.0) || !(st->r_obs > 0.0)) { set_error("state image-plane fields are not initialised (call gray_init_rays first)"); return GRAY_ERR_ARG; }
   }

@@ -78,7 +78,7 @@ int gray_integrate_host(const void* x_in_host, const void* k_in_host, void* x_ou
     gray_state st;
     st.x_dev = S.x; st.k_dev = S.k; st.status_dev = S.status; st.steps_dev = S.steps;
     st.n = m; st.prec = prec; st.pixels = GRAY_PIXELS_GRID;
-    st.a = a; st.r_obs = r_obs; st.inc_deg = 0; st.half_width = 0; st.nx = st.ny = 0; st.seed = 0; st.p0 = lo;
+    st.a = a; st.r_obs = r_obs; st.inc_deg = 0; st.half_width = 0; st.nx = st.ny = 0; st.seed = 0; st.p0 = lo; st.r_lo = 0; st.resume_dev = nullptr;
     rc = gray_integrate(&st, m, max_steps, params, S.ws, sizeof(Workspace), S.stream);
     if (rc) break;
     e = cudaMemcpyAsync((char*)x_out_host + lo * vec, S.x, m * vec, cudaMemcpyDeviceToHost, S.stream);

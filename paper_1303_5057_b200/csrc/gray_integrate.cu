@@ -16,6 +16,14 @@ template <typename S> struct Vec4T;
 template <> struct Vec4T<float> { using type = float4; };
 template <> struct Vec4T<double> { using type = double4; };
 
+// Resume records (gray_state.resume_dev, gray.h): integers and bit patterns travel in scalar slots of the batch's
+// precision; they are only loaded, stored and compared, never computed with.
+__device__ __forceinline__ float bits_to_scalar(unsigned long long b, float) { return __uint_as_float((unsigned int)b); }
+__device__ __forceinline__ double bits_to_scalar(unsigned long long b, double) { return __longlong_as_double((long long)b); }
+__device__ __forceinline__ unsigned long long scalar_bits(float v) { return __float_as_uint(v); }
+__device__ __forceinline__ unsigned long long scalar_bits(double v) { return (unsigned long long)__double_as_longlong(v); }
+constexpr unsigned long long kResumeMagic = 0x47524159ull;       // "GRAY"
+
 template <typename V>
 struct IntegrateArgs {
   using S = typename VT<V>::S;
@@ -23,6 +31,7 @@ struct IntegrateArgs {
   typename Vec4T<S>::type* k;
   uint8_t* status;
   uint32_t* steps;
+  typename Vec4T<S>::type* resume;   // gray_state.resume_dev: 4 vectors per photon, or NULL
   unsigned long long n;
   uint32_t max_steps;
   int refill_interval;
@@ -99,13 +108,35 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
       ys[4][l] = kv.x; ys[5][l] = kv.y; ys[6][l] = kh; ys[7][l] = kv.w;
 #pragma unroll
       for (int i = 0; i < 8; ++i) cs[i][l] = S(0);
+      // A photon left LIVE by an earlier call that wrote a resume record (gray.h): if the record belongs to exactly
+      // this stored state (same r, theta bits, same step count), the kernel's own variables - d, the folded theta,
+      // the compensation terms, E and L of the reduced system - are taken from it, and the continuation is
+      // bit-identical to an uninterrupted run.  Otherwise they are rebuilt from (r, theta) as above.
+      bool resumed = false;
+      if (A.resume != nullptr) {
+        const typename Vec4T<S>::type r3 = A.resume[4 * p + 3];
+        if (scalar_bits(r3.x) == scalar_bits(xv.y) && scalar_bits(r3.y) == scalar_bits(xv.z) &&
+            scalar_bits(r3.z) == (unsigned long long)s && scalar_bits(r3.w) == kResumeMagic) {
+          const typename Vec4T<S>::type r0 = A.resume[4 * p], r1 = A.resume[4 * p + 1], r2 = A.resume[4 * p + 2];
+          const unsigned long long flags = scalar_bits(r2.w);
+          m = (int)(flags & 1ull);
+          ys[1][l] = r0.x; ys[2][l] = r0.y;
+          ys[6][l] = m ? sneg(kv.z) : kv.z;
+          cs[1][l] = r1.x; cs[2][l] = r1.y; cs[3][l] = r1.z; cs[4][l] = r1.w;
+          cs[5][l] = r2.x; cs[6][l] = r2.y; cs[7][l] = r2.z;
+          if (RED) { ys[4][l] = r0.z; ys[7][l] = r0.w; }
+          resumed = true;
+        }
+      }
       if (RED) {
         // reduced system: the slots of k^t, k^phi carry the constants E, L of the photon, their compensation
         // slots -a E, -a L (rk4_step_reduced)
-        S E, L;
-        killing_constants(vget(K.a, 0), vget(K.rp, 0), ys[1][l], th, kv.x, kv.w, E, L);
-        ys[4][l] = E; ys[7][l] = L;
-        cs[4][l] = vneg(vmul(vget(K.a, 0), E)); cs[7][l] = vneg(vmul(vget(K.a, 0), L));
+        if (!resumed) {
+          S E, L;
+          killing_constants(vget(K.a, 0), vget(K.rp, 0), ys[1][l], th, kv.x, kv.w, E, L);
+          ys[4][l] = E; ys[7][l] = L;
+        }
+        cs[4][l] = vneg(vmul(vget(K.a, 0), ys[4][l])); cs[7][l] = vneg(vmul(vget(K.a, 0), ys[7][l]));
       }
       mirrored[l] = m;
       idx[l] = p;
@@ -129,6 +160,17 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
     A.k[p] = kv;
     A.status[p] = (uint8_t)st;
     A.steps[p] = nst[l];
+    if (A.resume != nullptr && st == GRAY_LIVE) {
+      // resume record of a photon stopped at max_steps (read back by take()): the kernel's own variables, tagged with
+      // the stored (r, theta) bits and the step count they belong to
+      typename Vec4T<S>::type r0, r1, r2, r3;
+      r0.x = vget(y[1], l); r0.y = th; r0.z = RED ? vget(y[4], l) : S(0); r0.w = RED ? vget(y[7], l) : S(0);
+      r1.x = vget(comp[1], l); r1.y = vget(comp[2], l); r1.z = vget(comp[3], l); r1.w = RED ? S(0) : vget(comp[4], l);
+      r2.x = vget(comp[5], l); r2.y = vget(comp[6], l); r2.z = RED ? S(0) : vget(comp[7], l);
+      r2.w = bits_to_scalar(mirrored[l] ? 1ull : 0ull, S(0));
+      r3.x = xv.y; r3.y = xv.z; r3.z = bits_to_scalar((unsigned long long)nst[l], S(0)); r3.w = bits_to_scalar(kResumeMagic, S(0));
+      A.resume[4 * p] = r0; A.resume[4 * p + 1] = r1; A.resume[4 * p + 2] = r2; A.resume[4 * p + 3] = r3;
+    }
     c_steps += nst[l] - nst0[l];
     if (st == GRAY_LIVE) ++c_live; else ++c_done;
     have[l] = false;
@@ -224,7 +266,7 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
           for (int l = 0; l < N; ++l) {
             ++nst[l];
             const bool bad_or_captured = !(zz[l] == S(0) && rr[l] >= K.r_cap);
-            bool f = have[l] && (bad_or_captured || !(rr[l] <= K.r_esc) || nst[l] == A.max_steps);
+            bool f = have[l] && (bad_or_captured || !(rr[l] <= K.r_esc) || nst[l] >= A.max_steps);
             if (EQ && slow) {
               if (landing[l] == 2) f = have[l];                              // second Newton step done: on the plane
               else if (landing[l] == 1) { landing[l] = 2; f = false; }
@@ -349,6 +391,7 @@ static int integrate(const gray_state* st, uint64_t n, uint32_t max_steps, const
   A.k = (typename Vec4T<S>::type*)st->k_dev;
   A.status = st->status_dev;
   A.steps = st->steps_dev;
+  A.resume = (typename Vec4T<S>::type*)st->resume_dev;
   A.n = n;
   A.max_steps = max_steps;
   A.refill_interval = p->refill_interval > 0 ? p->refill_interval : 8;

@@ -28,7 +28,7 @@ class _State(C.Structure):
     _fields_ = [("x_dev", C.c_void_p), ("k_dev", C.c_void_p), ("status_dev", C.c_void_p), ("steps_dev", C.c_void_p),
                 ("n", C.c_uint64), ("prec", C.c_int32), ("pixels", C.c_int32), ("a", C.c_double),
                 ("r_obs", C.c_double), ("inc_deg", C.c_double), ("half_width", C.c_double), ("nx", C.c_int32),
-                ("ny", C.c_int32), ("seed", C.c_uint64), ("p0", C.c_uint64), ("r_lo", C.c_double)]
+                ("ny", C.c_int32), ("seed", C.c_uint64), ("p0", C.c_uint64), ("r_lo", C.c_double), ("resume_dev", C.c_void_p)]
 
 
 class _StepParams(C.Structure):
@@ -119,7 +119,7 @@ class PhotonBatch:
     """Caller-owned device buffers of a gray_state: x, k (n x 4), status (n, uint8), steps (n, int32 bits of
     a uint32) and the workspace.  Memory comes from torch; nothing else does."""
 
-    def __init__(self, n, prec=GRAY_F32, device="cuda"):
+    def __init__(self, n, prec=GRAY_F32, device="cuda", resumable=False):
         if not torch.cuda.is_available():
             raise GrayError("no CUDA device: libgray has no CPU path")
         dt = torch.float32 if prec == GRAY_F32 else torch.float64
@@ -129,8 +129,11 @@ class PhotonBatch:
         self.status = torch.empty((self.n,), dtype=torch.uint8, device=device)
         self.steps = torch.empty((self.n,), dtype=torch.int32, device=device)
         self.workspace = torch.zeros((gray_workspace_bytes(self.n),), dtype=torch.uint8, device=device)
+        # gray_state.resume_dev (include/gray.h): makes interrupted gray_integrate calls bit-identical to one call
+        self.resume = torch.empty((self.n, 16), dtype=dt, device=device) if resumable else None
         self.c = _State(self.x.data_ptr(), self.k.data_ptr(), self.status.data_ptr(), self.steps.data_ptr(),
-                        self.n, prec, 0, 0.0, 0.0, 0.0, 0.0, 0, 0, 0, 0, 0.0)
+                        self.n, prec, 0, 0.0, 0.0, 0.0, 0.0, 0, 0, 0, 0, 0.0,
+                        self.resume.data_ptr() if resumable else None)
 
     def set_image_plane(self, a, r_obs, inc_deg, half_width, nx=0, ny=0, seed=0, p0=0, pixels=PIXELS_GRID):
         """Describe the image plane without running gray_init_rays (for states uploaded by the caller)."""

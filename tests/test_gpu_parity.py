@@ -212,7 +212,7 @@ def test_integrate_f32_rel_rule_matches_fp64_oracle(a, inc, W, nx, ny, ppt):
     _rel_rule_f32_parity(a, y, st, n, ref, edge_band(a, inc, al, be), retrace)
 
 
-def test_schedules_intervals_and_resume_are_bit_identical():
+def test_schedules_intervals_and_packing_are_bit_identical():
     a, inc, W, nx, ny = 0.9, 60.0, 10.0, 96, 51
     outs = []
     for prec in (g.GRAY_F32, g.GRAY_F64):
@@ -241,25 +241,91 @@ def test_schedules_intervals_and_resume_are_bit_identical():
             outs_xi.append((b.x.clone(), b.k.clone(), b.status.clone(), b.steps.clone(), g.gray_integrate_counters(b)["fallback_steps"]))
         assert outs_xi[0][4] == outs_xi[1][4] > 0
         assert all(torch.equal(u.view(torch.uint8), v.view(torch.uint8)) for u, v in zip(outs_xi[0][:4], outs_xi[1][:4]))
-        # resume: 100 steps, then 250 more, then to the end == one uninterrupted call
-        b = g.PhotonBatch(nx * ny, prec)
+
+
+def _run_in_pieces(b, caps, **kw):
+    total = 0
+    for cap in caps:
+        g.gray_integrate(b, max_steps=cap, params=g.StepParams(rule=g.STEP_EQ2, **kw))
+        total += g.gray_integrate_counters(b)["photon_steps"]
+    return total
+
+
+@pytest.mark.parametrize("prec,kw", [(g.GRAY_F32, dict()), (g.GRAY_F32, dict(photons_per_thread=1)), (g.GRAY_F64, dict()),
+                                     (g.GRAY_F32, dict(xi_epsilon=1e-3)), (g.GRAY_F32, dict(system=g.SYS_REDUCED)),
+                                     (g.GRAY_F64, dict(system=g.SYS_REDUCED)), (g.GRAY_F32, dict(stop_at_equator=True))])
+def test_resumed_calls_are_bit_identical_with_resume_records(prec, kw):
+    # "bit-identical results for any steps_per_launch" (the paper's interactive mode takes a few steps per
+    # call, P:81 fn 5).  With gray_state.resume_dev the kernel's own variables survive the store / load round trip
+    # (gray.h), so 100 + 250 + rest, and fifty 20-step calls + rest, equal one uninterrupted call bit for bit - for
+    # the packed and the scalar fp32 kernels, fp64, the xi monitor, the reduced system and the projection.
+    a, inc, W, nx, ny = 0.9, 60.0, 10.0, 96, 51
+    if kw.get("system") == g.SYS_REDUCED:
+        nx = 90                                   # even: no pixel column on the spin axis (reading R20)
+    n = nx * ny
+    one = g.PhotonBatch(n, prec)
+    g.gray_init_rays(one, a, wl.R_OBS, inc, W, nx, ny)
+    g.gray_integrate(one, max_steps=wl.MAX_STEPS, params=g.StepParams(rule=g.STEP_EQ2, **kw))
+    base = (one.x, one.k, one.status, one.steps)
+    for caps in ((100, 350, wl.MAX_STEPS), tuple(range(20, 1001, 20)) + (wl.MAX_STEPS,)):
+        b = g.PhotonBatch(n, prec, resumable=True)
+        b.resume.fill_(float("nan"))               # the record buffer need not be initialised
         g.gray_init_rays(b, a, wl.R_OBS, inc, W, nx, ny)
-        total = 0
-        for cap in (100, 350, wl.MAX_STEPS):
-            g.gray_integrate(b, max_steps=cap, params=g.StepParams(rule=g.STEP_EQ2))
-            c = g.gray_integrate_counters(b)
-            total += c["photon_steps"]
-            if cap == 100:
-                assert c["photons_live"] == nx * ny and c["photon_steps"] == 100 * nx * ny
-                assert int(b.steps.min().item()) == 100 and g.gray_classify(b)[g.LIVE] == nx * ny
-        # A stored state is (t, r, theta, phi), the kernel's own variables are r - r_+ and theta folded into
-        # [0, pi/2] (gray.h): a store / load round trip rounds them once, so a resumed run agrees with the
-        # uninterrupted one to rounding error amplified along the ray, not bit for bit.
+        g.gray_integrate(b, max_steps=caps[0], params=g.StepParams(rule=g.STEP_EQ2, **kw))
+        c = g.gray_integrate_counters(b)
+        assert c["photons_live"] == n and c["photon_steps"] == caps[0] * n and g.gray_classify(b)[g.LIVE] == n
+        assert int(b.steps.min().item()) == caps[0]
+        total = c["photon_steps"] + _run_in_pieces(b, caps[1:], **kw)
         assert total == int(b.steps.sum().item())
-        same = (b.status == base[2]) & (b.steps == base[3])
-        assert same.float().mean().item() > 0.998
-        err = ((b.x - base[0]).abs() / base[0].abs().clamp(min=1.0))[same][:, 1:].max(dim=1).values
-        assert err.quantile(0.99).item() < (2e-4 if prec == g.GRAY_F32 else 1e-10)
+        cur = (b.x, b.k, b.status, b.steps)
+        assert all(torch.equal(u.view(torch.uint8), v.view(torch.uint8)) for u, v in zip(base, cur)), caps[:3]
+    # a record that no longer matches the stored state is ignored: after the caller edits r the photon is re-read
+    b = g.PhotonBatch(n, prec, resumable=True)
+    g.gray_init_rays(b, a, wl.R_OBS, inc, W, nx, ny)
+    g.gray_integrate(b, max_steps=100, params=g.StepParams(rule=g.STEP_EQ2, **kw))
+    b2 = g.PhotonBatch(n, prec)
+    for dst, src in ((b2.x, b.x), (b2.k, b.k), (b2.status, b.status), (b2.steps, b.steps)):
+        dst.copy_(src)
+    b2.set_image_plane(a, wl.R_OBS, inc, W, nx, ny)
+    for q in (b, b2):
+        q.x[:, 1] *= 1.0 + 2.0 ** -12
+        g.gray_integrate(q, max_steps=wl.MAX_STEPS, params=g.StepParams(rule=g.STEP_EQ2, **kw))
+    assert torch.equal(b.x.view(torch.uint8), b2.x.view(torch.uint8)) and torch.equal(b.steps, b2.steps)
+
+
+@pytest.mark.parametrize("prec", [g.GRAY_F32, g.GRAY_F64])
+def test_resumed_calls_without_records_stay_within_the_parity_tolerances(prec):
+    # Without resume_dev every interruption rounds r = d + r_h and theta once and (fp32) drops the compensation terms
+    # (gray.h; reading R22).  Bound, not bit-identity: after sixty interruptions (fifty 20-step calls, then
+    # ten 100-step calls) every ray more than 1 % from the critical curve ends with the status of the uninterrupted
+    # run and, at equal step count, within the north-star MAX tolerance of it - 1e-3 in fp32, 1e-9 in fp64 - and
+    # the fp32 result still meets the 1e-3 bound against the fp64 oracle.
+    a, inc, W, nx, ny = 0.9, 60.0, 10.0, 96, 51
+    n = nx * ny
+    f32 = prec == g.GRAY_F32
+    one = g.PhotonBatch(n, prec)
+    g.gray_init_rays(one, a, wl.R_OBS, inc, W, nx, ny)
+    g.gray_integrate(one, max_steps=wl.MAX_STEPS, params=g.StepParams(rule=g.STEP_EQ2))
+    y1, st1, n1 = gpu_state(one)
+    b = g.PhotonBatch(n, prec)
+    g.gray_init_rays(b, a, wl.R_OBS, inc, W, nx, ny)
+    caps = tuple(range(20, 1001, 20)) + tuple(range(1100, 2001, 100)) + (wl.MAX_STEPS,)
+    total = _run_in_pieces(b, caps)
+    y, st, ns = gpu_state(b)
+    assert total == ns.sum() and not np.any(st == g.LIVE)
+    al, be = grid_pixels(W, nx, ny)
+    band = edge_band(a, inc, al, be)
+    assert np.all((st == st1) | band)
+    same = (st == st1) & (ns == n1) & ~band
+    assert same[~band].mean() >= (0.99 if f32 else 0.999)      # a threshold crossed within rounding moves the count by one
+    err = rel_err_final(y[same], y1[same])
+    assert err.max() <= (1e-3 if f32 else 1e-9), err.max()
+    assert np.quantile(err, 0.99) <= (1e-4 if f32 else 1e-10), np.quantile(err, 0.99)
+    if f32:
+        ref = o.trace(a, wl.R_OBS, inc, W, nx, ny, rule=o.STEP_EQ2, init_f32=True, threads=8)
+        ok = (st == ref["status"]) & (ns == ref["steps"]) & ~band
+        assert ok[~band].mean() >= 0.98
+        assert rel_err_final(y[ok], ref["y"][ok]).max() <= 1e-3
 
 
 @pytest.mark.parametrize("prec", [g.GRAY_F32, g.GRAY_F64])
