@@ -229,7 +229,7 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
         if (!FROZEN) {
           bool rej[N];
           if (RED) rk4_step_reduced<RULE>(K, y, comp);
-          else rk4_step<XI>(K, y, comp, dl, rej);
+          else rk4_step<XI, RULE == GRAY_STEP_EQ2 && !EQ>(K, y, comp, dl, rej);
           if (XI) {
 #pragma unroll
             for (int l = 0; l < N; ++l) c_fallback += (rej[l] && have[l]) ? 1u : 0u;
@@ -295,7 +295,7 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
 #pragma unroll
           for (int i = 0; i < 8; ++i) { w[i] = y[i]; wc[i] = comp[i]; }
           bool rej[N];
-          rk4_step<false>(K, w, wc, dl, rej);
+          rk4_step<false, RULE == GRAY_STEP_EQ2>(K, w, wc, dl, rej);
           const V z = nonfinite_probe(K, w);
           const V r = w[1];
           S th[N], ph[N], kh[N], c2[N], c6[N];

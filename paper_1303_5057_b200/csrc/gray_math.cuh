@@ -48,6 +48,8 @@ struct Consts {
   V zero, one, mone, two, m2, half, nhalf, sixth, ninth;
   // sin / cos (float builds): quadrant reduction and minimax polynomials, see sincos_v
   V two_over_pi, magic, npio2_hi, npio2_lo, s1, s2, s3, c1, c2, c3, c4;
+  V fs1, fs2, fs3, fs4, fc1, fc2, fc3, fc4, fc5;   // sincos_folded (float builds)
+  V nsixth, r24;                                   // sincos_rotate (float builds): -1/6, 1/24
   S r_cap, r_esc;                         // termination radii, as heights above the horizon (r - r_+): the kernel's radial variable
   S xi_eps;                               // epsilon of the xi monitor (paper eq. 4); 0 = off
 };
@@ -68,6 +70,10 @@ __host__ inline Consts<V> make_consts(double a, double h, double r_cap, double r
   K.npio2_hi = B(-1.57079637050628662109375); K.npio2_lo = B(4.371139000186241e-08);
   K.s1 = B(-1.666666418e-01); K.s2 = B(8.332700469e-03); K.s3 = B(-1.957778732e-04);
   K.c1 = B(-0.5); K.c2 = B(4.166664928e-02); K.c3 = B(-1.388748409e-03); K.c4 = B(2.445036807e-05);
+  K.fs1 = B(-1.6666642594e-01); K.fs2 = B(8.3326730771e-03); K.fs3 = B(-1.9783720104e-04); K.fs4 = B(2.5544161709e-06);
+  K.fc1 = B(-4.9999998057e-01); K.fc2 = B(4.1666583344e-02); K.fc3 = B(-1.3887727202e-03); K.fc4 = B(2.4730754562e-05);
+  K.fc5 = B(-2.5585777763e-07);
+  K.nsixth = B(-1.0 / 6.0); K.r24 = B(1.0 / 24.0);
   K.r_cap = (S)(r_cap - (1.0 + root)); K.r_esc = (S)(r_esc - (1.0 + root));   // differences formed in double
   return K;
 }
@@ -139,15 +145,93 @@ GRAY_DEV void sincos_v<double>(const Consts<double>&, double x, double& s, doubl
   c = ((j + 1) & 2) ? -cc : cc;                                 // quadrants 1, 2: cos < 0
 }
 
-// ---- right-hand side: accelerations dk^mu/dlambda at (d = r - r_+, th) for momentum (kt, kr, kh, kp) ----
+// ---- sin and cos inside one RK4 step ---------------------------------------------------------------------
+// The four right-hand sides of a step are evaluated at th0 (stage 1) and at th0 + dlt with small dlt (stages 2-4:
+// dlt = dlambda/2 k^th or dlambda k^th, and eq. (2) keeps |dlambda k^th| <= h).  So only stage 1 needs a sine and
+// a cosine of an angle; the others follow by the angle-addition formulas from (s0, c0) and the Taylor series of
+// sin, cos of dlt, which needs no range reduction, no quadrant logic and fewer operations.
+//
+// sincos_folded, float builds: x is the kernel's folded polar angle, in [0, pi/2] at the start of every step
+// (remap_theta) - fitted polynomials on [-0.25, pi/2 + 0.25] (sin: odd, relative error 2.8e-8; cos: even, absolute
+// error 1.4e-9), 11 FP-pipe operations and no integer / select work at all.  The double build keeps sincos_v.
+template <typename V>
+GRAY_DEV void sincos_folded(const Consts<V>& K, V x, V& s, V& c) {
+  const V u = vmul(x, x);
+  const V sp = vfma(vfma(vfma(K.fs4, u, K.fs3), u, K.fs2), u, K.fs1);
+  s = vfma(vmul(x, u), sp, x);
+  const V cp = vfma(vfma(vfma(vfma(K.fc5, u, K.fc4), u, K.fc3), u, K.fc2), u, K.fc1);
+  c = vfma(u, cp, K.one);
+}
+template <>
+GRAY_DEV void sincos_folded<double>(const Consts<double>& K, double x, double& s, double& c) { sincos_v(K, x, s, c); }
+
+// (s, c) = (sin, cos)(th0 + dlt) from (s0, c0) = (sin, cos)(th0):  s = s0 + c0 sd + s0 cm,  c = c0 - s0 sd + c0 cm
+// with sd = sin(dlt), cm = cos(dlt) - 1 by their Taylor series.  float: sd = dlt - dlt^3/6, cm = -dlt^2/2 + dlt^4/24
+// (9 operations; truncation < 3.4e-8 relative for |dlt| <= kRotateMax).  double: through dlt^9 / dlt^10
+// (15 operations; < 3e-17 for |dlt| <= 1/8).
+template <typename S> struct RotateMax;
+template <> struct RotateMax<float> { static constexpr float value = 0.045f; };
+template <> struct RotateMax<double> { static constexpr double value = 0.125; };
+template <typename V>
+GRAY_DEV void sincos_rotate(const Consts<V>& K, V s0, V c0, V dlt, V& s, V& c) {
+  const V u = vmul(dlt, dlt);
+  const V sd = vfma(vmul(dlt, u), K.nsixth, dlt);
+  const V cm = vmul(u, vfma(u, K.r24, K.nhalf));
+  s = vfma(s0, cm, vfma(c0, sd, s0));
+  c = vfma(c0, cm, vfma(s0, vneg(sd), c0));
+}
+template <>
+GRAY_DEV void sincos_rotate<double>(const Consts<double>&, double s0, double c0, double dlt, double& s, double& c) {
+  const double u = __dmul_rn(dlt, dlt);
+  double sp = 2.7557319223985890653e-06;                        //  1/9!
+  sp = __fma_rn(sp, u, -1.9841269841269841270e-04);             // -1/7!
+  sp = __fma_rn(sp, u, 8.3333333333333332177e-03);              //  1/5!
+  sp = __fma_rn(sp, u, -1.6666666666666665741e-01);             // -1/3!
+  const double sd = __fma_rn(__dmul_rn(dlt, u), sp, dlt);
+  double cp = -2.7557319223985888276e-07;                       // -1/10!
+  cp = __fma_rn(cp, u, 2.4801587301587301566e-05);              //  1/8!
+  cp = __fma_rn(cp, u, -1.3888888888888889419e-03);             // -1/6!
+  cp = __fma_rn(cp, u, 4.1666666666666664354e-02);              //  1/4!
+  cp = __fma_rn(cp, u, -0.5);
+  const double cm = __dmul_rn(u, cp);
+  s = __fma_rn(s0, cm, __fma_rn(c0, sd, s0));
+  c = __fma_rn(c0, cm, __fma_rn(-s0, sd, c0));
+}
+// One photon whose stage offset is outside the series' range (a large k^th next to the axis, or a step rule
+// without an angular limit: rare): sine and cosine of th0 + dlt from the CUDA math library.  Kept out of line so that
+// its constants and slow path cost the loop nothing.
+__device__ __noinline__ float2 sincos_wide(float th0, float dlt) { float2 r; sincosf(__fadd_rn(th0, dlt), &r.x, &r.y); return r; }
+__device__ __noinline__ double2 sincos_wide(double th0, double dlt) { double2 r; sincos(__dadd_rn(th0, dlt), &r.x, &r.y); return r; }
+// sine and cosine of th0 + dlt for a stage, from (s0, c0) = (sin, cos)(th0).  Each photon by its own |dlt| (its
+// result must not depend on the photon it shares a thread with): the rotation within the series' range, else
+// sincos_wide.  A NaN dlt stays NaN.
+template <typename V>
+GRAY_DEV void sincos_stage(const Consts<V>& K, V th0, V s0, V c0, V dlt, V& s, V& c) {
+  using S = typename VT<V>::S;
+  constexpr int N = VT<V>::N;
+  S a[N];
+  vunpack(dlt, a);
+  bool wide = false;
+#pragma unroll
+  for (int l = 0; l < N; ++l) wide |= !(sabs(a[l]) <= RotateMax<S>::value);
+  sincos_rotate(K, s0, c0, dlt, s, c);
+  if (wide) {
+    S sr[N], cr[N], tb[N];
+    vunpack(s, sr); vunpack(c, cr); vunpack(th0, tb);
+#pragma unroll
+    for (int l = 0; l < N; ++l)
+      if (!(sabs(a[l]) <= RotateMax<S>::value)) { const auto sc = sincos_wide(tb[l], a[l]); sr[l] = sc.x; cr[l] = sc.y; }
+    vpack(s, sr); vpack(c, cr);
+  }
+}
+
+// ---- right-hand side: accelerations dk^mu/dlambda at d = r - r_+, (s, c) = (sin, cos)(theta) for momentum (kt, kr, kh, kp) ----
 // out[i] = dk^i/dlambda (i = t, r, th, phi) if !ACC, else add[i] + dk^i/dlambda with the addition fused into the
 // last multiply of each component (stage 4 of RK4 needs only that sum).  No addition or subtraction below
 // takes a single-use product as an operand: ptxas contracts such pairs of packed instructions into FFMA2
 // even though both carry .rn, which would make the f2 build round differently from the float build.
 template <bool ACC, typename V>
-GRAY_DEV void geodesic_accel(const Consts<V>& K, V d, V th, V kt, V kr, V kh, V kp, const V* add, V out[4]) {
-  V s, c;
-  sincos_v(K, th, s, c);
+GRAY_DEV void geodesic_accel(const Consts<V>& K, V d, V s, V c, V kt, V kr, V kh, V kp, const V* add, V out[4]) {
   const V r = vadd(d, K.rp);
   const V r2 = vmul(r, r);
   const V c2 = vmul(c, c);
@@ -258,40 +342,46 @@ GRAY_DEV void null_norm(const Consts<V>& K, const V y[8], V& Nn, V& Dn) {
 // XI: the paper's production pole treatment: if the state the RK4 step produced has |xi + 1| > epsilon
 // (or a non-finite xi), the step is re-integrated from the old state as one forward Euler step of dlambda / 9,
 // which is not tested itself.  rejected[l] reports it per photon.
-template <bool XI, typename V>
+// FOLDED: y[2] is known to lie in the range of sincos_folded (the kernel's folded theta under the eq. (2) rule).
+template <bool XI, bool FOLDED, typename V>
 GRAY_DEV void rk4_step(const Consts<V>& K, V y[8], V comp[8], V dl, bool rejected[VT<V>::N]) {
   using S = typename VT<V>::S;
   constexpr int N = VT<V>::N;
   V acc[8], w[8], f[4], f1[4];
   const V hdl = vmul(K.half, dl);
   // stage 1
-  geodesic_accel<false>(K, y[1], y[2], y[4], y[5], y[6], y[7], (const V*)nullptr, f);
+  V s0, c0, ss, cc;
+  if (FOLDED) sincos_folded(K, y[2], s0, c0);
+  else sincos_v(K, y[2], s0, c0);
+  geodesic_accel<false>(K, y[1], s0, c0, y[4], y[5], y[6], y[7], (const V*)nullptr, f);
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
     f1[i] = f[i];
     acc[i] = y[4 + i];
     acc[4 + i] = f[i];
-    w[i] = vfma(hdl, y[4 + i], y[i]);
+    w[i] = i == 2 ? vmul(hdl, y[6]) : vfma(hdl, y[4 + i], y[i]);      // w[2]: the stage's offset in theta, not theta
     w[4 + i] = vfma(hdl, f[i], y[4 + i]);
   }
   // stages 2 and 3
 #pragma unroll
   for (int stage = 2; stage <= 3; ++stage) {
     const V hs = stage == 2 ? hdl : dl;
-    geodesic_accel<false>(K, w[1], w[2], w[4], w[5], w[6], w[7], (const V*)nullptr, f);
+    sincos_stage(K, y[2], s0, c0, w[2], ss, cc);
+    geodesic_accel<false>(K, w[1], ss, cc, w[4], w[5], w[6], w[7], (const V*)nullptr, f);
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
       const V kx = w[4 + i];
       acc[i] = vfma(K.two, kx, acc[i]);
       acc[4 + i] = vfma(K.two, f[i], acc[4 + i]);
-      w[i] = vfma(hs, kx, y[i]);
+      w[i] = i == 2 ? vmul(hs, kx) : vfma(hs, kx, y[i]);
       w[4 + i] = vfma(hs, f[i], y[4 + i]);
     }
   }
   // stage 4: the sums k1 + 2 k2 + 2 k3 + k4
 #pragma unroll
   for (int i = 0; i < 4; ++i) acc[i] = vadd(acc[i], w[4 + i]);
-  geodesic_accel<true>(K, w[1], w[2], w[4], w[5], w[6], w[7], acc + 4, acc + 4);
+  sincos_stage(K, y[2], s0, c0, w[2], ss, cc);
+  geodesic_accel<true>(K, w[1], ss, cc, w[4], w[5], w[6], w[7], acc + 4, acc + 4);
   V yn[8], cn[8];
   advance_state(y, comp, vmul(K.sixth, dl), acc, yn, cn);
 #pragma unroll
@@ -369,10 +459,8 @@ GRAY_DEV void killing_velocities(S a, S rp, S rpm, S d, S th, S E, S L, S& kt, S
 
 // accelerations of (k^r, k^theta) -> out[0], out[1] (ACC: added to add[0], add[1]); k^t, k^phi of the point -> kt, kp
 template <bool ACC, typename V>
-GRAY_DEV void geodesic_accel_reduced(const Consts<V>& K, V d, V th, V kr, V kh, V E, V L, V naE, V naL, const V* add,
+GRAY_DEV void geodesic_accel_reduced(const Consts<V>& K, V d, V s, V c, V kr, V kh, V E, V L, V naE, V naL, const V* add,
                                      V out[2], V& kt, V& kp) {
-  V s, c;
-  sincos_v(K, th, s, c);
   const V r = vadd(d, K.rp);
   const V r2 = vmul(r, r);
   const V c2 = vmul(c, c);
@@ -414,24 +502,28 @@ GRAY_DEV void geodesic_accel_reduced(const Consts<V>& K, V d, V th, V kr, V kh, 
 template <int RULE, typename V>
 GRAY_DEV void rk4_step_reduced(const Consts<V>& K, V y[8], V comp[8]) {
   const V E = y[4], L = y[7], naE = comp[4], naL = comp[7];
-  V f[2], kt, kp, acc[8], w1, w2, w5, w6;
-  geodesic_accel_reduced<false>(K, y[1], y[2], y[5], y[6], E, L, naE, naL, (const V*)nullptr, f, kt, kp);
+  V f[2], kt, kp, acc[8], w1, w2, w5, w6, s0, c0, ss, cc;
+  if (RULE == 1) sincos_folded(K, y[2], s0, c0);
+  else sincos_v(K, y[2], s0, c0);
+  geodesic_accel_reduced<false>(K, y[1], s0, c0, y[5], y[6], E, L, naE, naL, (const V*)nullptr, f, kt, kp);
   const V dl = step_size<V, RULE>(K, y[1], y[5], y[6], kp);
   const V hdl = vmul(K.half, dl);
   acc[0] = kt; acc[3] = kp; acc[1] = y[5]; acc[2] = y[6]; acc[5] = f[0]; acc[6] = f[1];
-  w1 = vfma(hdl, y[5], y[1]); w2 = vfma(hdl, y[6], y[2]); w5 = vfma(hdl, f[0], y[5]); w6 = vfma(hdl, f[1], y[6]);
+  w1 = vfma(hdl, y[5], y[1]); w2 = vmul(hdl, y[6]); w5 = vfma(hdl, f[0], y[5]); w6 = vfma(hdl, f[1], y[6]);   // w2: offset in theta
 #pragma unroll
   for (int stage = 2; stage <= 3; ++stage) {
     const V hs = stage == 2 ? hdl : dl;
-    geodesic_accel_reduced<false>(K, w1, w2, w5, w6, E, L, naE, naL, (const V*)nullptr, f, kt, kp);
+    sincos_stage(K, y[2], s0, c0, w2, ss, cc);
+    geodesic_accel_reduced<false>(K, w1, ss, cc, w5, w6, E, L, naE, naL, (const V*)nullptr, f, kt, kp);
     acc[0] = vfma(K.two, kt, acc[0]); acc[3] = vfma(K.two, kp, acc[3]);
     acc[1] = vfma(K.two, w5, acc[1]); acc[2] = vfma(K.two, w6, acc[2]);
     acc[5] = vfma(K.two, f[0], acc[5]); acc[6] = vfma(K.two, f[1], acc[6]);
     const V k5 = w5, k6 = w6;
-    w1 = vfma(hs, k5, y[1]); w2 = vfma(hs, k6, y[2]); w5 = vfma(hs, f[0], y[5]); w6 = vfma(hs, f[1], y[6]);
+    w1 = vfma(hs, k5, y[1]); w2 = vmul(hs, k6); w5 = vfma(hs, f[0], y[5]); w6 = vfma(hs, f[1], y[6]);
   }
   acc[1] = vadd(acc[1], w5); acc[2] = vadd(acc[2], w6);
-  geodesic_accel_reduced<true>(K, w1, w2, w5, w6, E, L, naE, naL, acc + 5, acc + 5, kt, kp);
+  sincos_stage(K, y[2], s0, c0, w2, ss, cc);
+  geodesic_accel_reduced<true>(K, w1, ss, cc, w5, w6, E, L, naE, naL, acc + 5, acc + 5, kt, kp);
   acc[0] = vadd(acc[0], kt); acc[3] = vadd(acc[3], kp);
   const V dl6 = vmul(K.sixth, dl);
 #pragma unroll
