@@ -291,38 +291,39 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
             for (int l = 0; l < N; ++l) lnd |= landing[l] != 0;
           }
         } else {
-          V w[8], wc[8];
-#pragma unroll
-          for (int i = 0; i < 8; ++i) { w[i] = y[i]; wc[i] = comp[i]; }
-          bool rej[N];
-          rk4_step<false, RULE == GRAY_STEP_EQ2>(K, w, wc, dl, rej);
-          const V z = nonfinite_probe(K, w);
-          const V r = w[1];
-          S th[N], ph[N], kh[N], c2[N], c6[N];
-          int wm[N];
+          // Peak-rate case (gray.h `frozen`): every slot executes the whole step; a slot whose photon has finished
+          // takes it with dlambda = 0 (no stage leaves its state) and its increments are replaced by its own
+          // residuals, so its state stays exactly as it is whatever the right-hand sides evaluate to there.
           bool adv[N];
-          vunpack(w[2], th); vunpack(w[3], ph); vunpack(w[6], kh); vunpack(wc[2], c2); vunpack(wc[6], c6);
+          S dls[N];
+          vunpack(dl, dls);
 #pragma unroll
           for (int l = 0; l < N; ++l) {
-            wm[l] = mirrored[l];
-            remap_theta(th[l], ph[l], kh[l], c2[l], c6[l], wm[l], true);
             adv[l] = have[l] && fstat[l] == GRAY_LIVE;
+            dls[l] = adv[l] ? dls[l] : S(0);
           }
-          vpack(w[2], th); vpack(w[3], ph); vpack(w[6], kh); vpack(wc[2], c2); vpack(wc[6], c6);
-          // frozen by select: a slot advances only while its photon is live
+          vpack(dl, dls);
+          bool rej[N];
+          rk4_step<false, false, true>(K, y, comp, dl, rej, adv);
+          const V z = nonfinite_probe(K, y);
+          const V r = y[1];
+          S th[N], zz[N], rr[N];
+          vunpack(y[2], th); vunpack(z, zz); vunpack(r, rr);
+          bool out_of_fold = false;
 #pragma unroll
-          for (int i = 0; i < 8; ++i) {
-            S a[N], b[N], ca[N], cb[N];
-            vunpack(y[i], a); vunpack(w[i], b); vunpack(comp[i], ca); vunpack(wc[i], cb);
+          for (int l = 0; l < N; ++l) out_of_fold |= adv[l] && !(th[l] >= S(0) && th[l] <= S(1.57079632679489661923));
+          if (out_of_fold) {
+            S ph[N], kh[N], c2[N], c6[N];
+            vunpack(y[3], ph); vunpack(y[6], kh); vunpack(comp[2], c2); vunpack(comp[6], c6);
 #pragma unroll
-            for (int l = 0; l < N; ++l) { a[l] = adv[l] ? b[l] : a[l]; ca[l] = adv[l] ? cb[l] : ca[l]; }
-            vpack(y[i], a); vpack(comp[i], ca);
+            for (int l = 0; l < N; ++l)
+              if (adv[l]) remap_theta(th[l], ph[l], kh[l], c2[l], c6[l], mirrored[l], true);
+            vpack(y[2], th); vpack(y[3], ph); vpack(y[6], kh); vpack(comp[2], c2); vpack(comp[6], c6);
           }
 #pragma unroll
           for (int l = 0; l < N; ++l) {
             if (have[l]) {
-              const int st = state_status(vget(z, l), vget(r, l), K.r_cap, K.r_esc);
-              mirrored[l] = adv[l] ? wm[l] : mirrored[l];
+              const int st = state_status(zz[l], rr[l], K.r_cap, K.r_esc);
               nst[l] += adv[l] ? 1u : 0u;
               fstat[l] = adv[l] ? st : fstat[l];
               ++iss[l];

@@ -204,7 +204,7 @@ __device__ __noinline__ float2 sincos_wide(float th0, float dlt) { float2 r; sin
 __device__ __noinline__ double2 sincos_wide(double th0, double dlt) { double2 r; sincos(__dadd_rn(th0, dlt), &r.x, &r.y); return r; }
 // sine and cosine of th0 + dlt for a stage, from (s0, c0) = (sin, cos)(th0).  Each photon by its own |dlt| (its
 // result must not depend on the photon it shares a thread with): the rotation within the series' range, else
-// sincos_wide.  A NaN dlt stays NaN.
+// sincos_wide.  A NaN dlt goes through the rotation and comes out NaN.
 template <typename V>
 GRAY_DEV void sincos_stage(const Consts<V>& K, V th0, V s0, V c0, V dlt, V& s, V& c) {
   using S = typename VT<V>::S;
@@ -213,14 +213,14 @@ GRAY_DEV void sincos_stage(const Consts<V>& K, V th0, V s0, V c0, V dlt, V& s, V
   vunpack(dlt, a);
   bool wide = false;
 #pragma unroll
-  for (int l = 0; l < N; ++l) wide |= !(sabs(a[l]) <= RotateMax<S>::value);
+  for (int l = 0; l < N; ++l) wide |= sabs(a[l]) > RotateMax<S>::value;
   sincos_rotate(K, s0, c0, dlt, s, c);
   if (wide) {
     S sr[N], cr[N], tb[N];
     vunpack(s, sr); vunpack(c, cr); vunpack(th0, tb);
 #pragma unroll
     for (int l = 0; l < N; ++l)
-      if (!(sabs(a[l]) <= RotateMax<S>::value)) { const auto sc = sincos_wide(tb[l], a[l]); sr[l] = sc.x; cr[l] = sc.y; }
+      if (sabs(a[l]) > RotateMax<S>::value) { const auto sc = sincos_wide(tb[l], a[l]); sr[l] = sc.x; cr[l] = sc.y; }
     vpack(s, sr); vpack(c, cr);
   }
 }
@@ -298,8 +298,11 @@ GRAY_DEV V step_size(const Consts<V>& K, V d, V kr, V kh, V kp) {
 // ---- state update y <- y + scale * rate --------------------------------------------------------------
 // `comp` carries, for the float builds, the rounding error of each update into the next one (compensated
 // summation): y + comp is the state to roughly twice the working precision.
-template <typename V>
-GRAY_DEV void advance_state(const V y[8], const V comp[8], V scale, const V rate[8], V yn[8], V cn[8]) {
+template <bool MASKED = false, typename V>
+GRAY_DEV void advance_state(const V y[8], const V comp[8], V scale, const V rate[8], V yn[8], V cn[8],
+                            const bool* adv = nullptr) {
+  using S = typename VT<V>::S;
+  constexpr int N = VT<V>::N;
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
     if (sizeof(typename VT<V>::S) == 4 && ((GRAY_COMP_MASK >> i) & 1)) {
@@ -307,8 +310,23 @@ GRAY_DEV void advance_state(const V y[8], const V comp[8], V scale, const V rate
       const V s = vadd(y[i], inc);
       cn[i] = vsub(inc, vsub(s, y[i]));        // Fast2Sum: exact whenever |y| >= |inc|
       yn[i] = s;
+      if (MASKED) {
+        // a slot that does not advance keeps its value and its residual, whatever (finite or not) its rate came out as
+        S a[N], b[N], ca[N], cb[N];
+        vunpack(yn[i], a); vunpack(y[i], b); vunpack(cn[i], ca); vunpack(comp[i], cb);
+#pragma unroll
+        for (int l = 0; l < N; ++l) { a[l] = adv[l] ? a[l] : b[l]; ca[l] = adv[l] ? ca[l] : cb[l]; }
+        vpack(yn[i], a); vpack(cn[i], ca);
+      }
     } else {
       yn[i] = vfma(scale, rate[i], y[i]);
+      if (MASKED) {
+        S a[N], b[N];
+        vunpack(yn[i], a); vunpack(y[i], b);
+#pragma unroll
+        for (int l = 0; l < N; ++l) a[l] = adv[l] ? a[l] : b[l];
+        vpack(yn[i], a);
+      }
       cn[i] = comp[i];
     }
   }
@@ -343,8 +361,10 @@ GRAY_DEV void null_norm(const Consts<V>& K, const V y[8], V& Nn, V& Dn) {
 // (or a non-finite xi), the step is re-integrated from the old state as one forward Euler step of dlambda / 9,
 // which is not tested itself.  rejected[l] reports it per photon.
 // FOLDED: y[2] is known to lie in the range of sincos_folded (the kernel's folded theta under the eq. (2) rule).
-template <bool XI, bool FOLDED, typename V>
-GRAY_DEV void rk4_step(const Consts<V>& K, V y[8], V comp[8], V dl, bool rejected[VT<V>::N]) {
+// MASKED (gray.h `frozen`): only the slots with adv[l] advance; the others keep their state bit for bit while the
+// arithmetic of the step is carried out for them all the same (the caller passes them dlambda = 0).
+template <bool XI, bool FOLDED, bool MASKED = false, typename V>
+GRAY_DEV void rk4_step(const Consts<V>& K, V y[8], V comp[8], V dl, bool rejected[VT<V>::N], const bool* adv = nullptr) {
   using S = typename VT<V>::S;
   constexpr int N = VT<V>::N;
   V acc[8], w[8], f[4], f1[4];
@@ -383,7 +403,7 @@ GRAY_DEV void rk4_step(const Consts<V>& K, V y[8], V comp[8], V dl, bool rejecte
   sincos_stage(K, y[2], s0, c0, w[2], ss, cc);
   geodesic_accel<true>(K, w[1], ss, cc, w[4], w[5], w[6], w[7], acc + 4, acc + 4);
   V yn[8], cn[8];
-  advance_state(y, comp, vmul(K.sixth, dl), acc, yn, cn);
+  advance_state<MASKED>(y, comp, vmul(K.sixth, dl), acc, yn, cn, adv);
 #pragma unroll
   for (int l = 0; l < N; ++l) rejected[l] = false;
   if (XI) {
