@@ -334,10 +334,9 @@ GRAY_DEV void advance_state(const V y[8], const V comp[8], V scale, const V rate
 
 // ---- the paper's xi (eq. 4): N = g_mu_nu k^mu k^nu and D = g_tt (k^t)^2, xi + 1 = N / D ---------------
 //   N = -(k^t)^2 + (2r/Sigma) u^2 + Sigma ((k^r)^2/Delta + (k^th)^2) + rho s^2 (k^phi)^2,  D = (2r/Sigma - 1) (k^t)^2
+// (s, c) = (sin, cos)(y[2]), supplied by the caller.
 template <typename V>
-GRAY_DEV void null_norm(const Consts<V>& K, const V y[8], V& Nn, V& Dn) {
-  V s, c;
-  sincos_v(K, y[2], s, c);
+GRAY_DEV void null_norm(const Consts<V>& K, const V y[8], V s, V c, V& Nn, V& Dn) {
   const V d = y[1], kt = y[4], kr = y[5], kh = y[6], kp = y[7];
   const V r = vadd(d, K.rp);
   const V r2 = vmul(r, r);
@@ -407,8 +406,11 @@ GRAY_DEV void rk4_step(const Consts<V>& K, V y[8], V comp[8], V dl, bool rejecte
 #pragma unroll
   for (int l = 0; l < N; ++l) rejected[l] = false;
   if (XI) {
-    V Nn, Dn;
-    null_norm(K, yn, Nn, Dn);
+    // sine and cosine at the new state: (s0, c0) turned by the step's own increment of theta (yn[2] and y[2] differ by
+    // it up to the rounding the compensation carries)
+    V Nn, Dn, sn, cn2;
+    sincos_stage(K, y[2], s0, c0, vsub(yn[2], y[2]), sn, cn2);
+    null_norm(K, yn, sn, cn2, Nn, Dn);
     S nn[N], dn[N];
     vunpack(Nn, nn); vunpack(Dn, dn);
     bool any = false;
