@@ -31,13 +31,9 @@ FLOPS_PER_PHOTON_STEP = {"rel": 777, "eq2": 787}
 # FP32 CUDA-core peak the integrator is bound by: 148 SMs x 128 lanes x 2 (FMA) x
 # 1.965 GHz (clocks.max.sm); FP64: 64 lanes per SM.
 PEAK_TFLOPS = {"f32": 148 * 128 * 2 * 1.965e9 / 1e12, "f64": 148 * 64 * 2 * 1.965e9 / 1e12}
-# dram__bytes_read.sum + dram__bytes_write.sum of one gray_integrate launch of the default workload (2^30 photons,
-# fp32) from the committed ncu capture profiles/r01_integrate_f2_dram_2p30.csv: 40.217 GB + 39.874 GB, per photon
-NCU_DRAM_BYTES_PER_PHOTON = 74.59
-# FP32 operations the packed kernel EXECUTES per photon-step (FMA = 2), from the instruction counts of the committed
-# ncu capture (profiles/r01_README.md: FFMA2 166.4, FMUL2 179.4, FADD2 51.1 per warp per step of its 64 photons, plus
-# scalar FADD): fewer than the oracle's tally because the kernel contracts the Christoffel sums analytically
-NCU_EXECUTED_FLOPS_PER_PHOTON_STEP = 563
+# The survey's own hand count of a photon-step in the collected-term formulation (655 + 8 trig),
+# a third reading next to the oracle's tally and the executed count
+FLOPS_SURVEY_HAND_TALLY = 663
 
 
 def parse():
@@ -58,7 +54,10 @@ def parse():
     ap.add_argument("--photons-per-thread", type=int, default=0, help="0 = library default (2 for f32: packed FFMA2), 1, 2")
     ap.add_argument("--system", default="full", choices=["full", "reduced"], help="full = the 8 second-order equations of the north star; reduced = E, L_z eliminate k^t, k^phi")
     ap.add_argument("--xi-eps", type=float, default=0.0, help="epsilon of the paper's xi monitor (P:107); 0 = off")
-    ap.add_argument("--e2e-log2n", type=int, default=-1, help="photons per GPU of the host-buffer run (default min(log2n, 26))")
+    ap.add_argument("--e2e-log2n", type=int, default=-1, help="photons per GPU of the host-buffer run (default min(log2n, 28), lowered if the host "
+                    "cannot pin the buffers)")
+    ap.add_argument("--no-secondary", action="store_true", help="skip the secondary measurements (C4 sweep, peak case, fp64, xi, reduced)")
+    ap.add_argument("--cpu-log2n", type=int, default=21, help="photons of the oracle's all-core sample (the one-core sample has 1/16 of it)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--dist-backend", default="nccl", help="torch.distributed backend of the N > 1 run (the data path has no "
                     "collective; only the timing / counter reduction uses it)")
@@ -160,201 +159,353 @@ def run_reference(args):
     out = {"impl": "reference", "metric": "photon-steps/s", "value": value, "unit": "photon-steps/s", "n_gpus": args.gpus,
            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps, "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-           "config": workload_config(args, 1), "ns_per_photon_step": 1e9 / value,
+           "config": dict(workload_config(args, 1), precision="f64 (the oracle's arithmetic; the GPU arm's is f32)"),
+           "ns_per_photon_step": 1e9 / value,
            "cpu_baseline": {"value": value, "unit": "photon-steps/s", "cores": threads, "kind": "oracle", "sample": sample},
            "e2e": {"value": value, "unit": "photon-steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
            "gpu_launches": 0}
     print(json.dumps(out), flush=True)
 
 
-def run_gray(args):
-    import torch
-    import torch.distributed as dist
+def read_profile_csv(name):
+    """Rows of a committed ncu CSV under profiles/ (lines before the header are ncu's own banner)."""
+    import csv
+    path = os.path.join(ROOT, "profiles", name)
+    if not os.path.exists(path):
+        return None
+    with open(path) as f:
+        lines = [l for l in f if l.startswith('"')]
+    return list(csv.DictReader(lines))
 
-    import paper_1303_5057_b200 as g
-    from paper_1303_5057_b200 import workloads as wl
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device (libgray has no CPU path)")
-    if args.share_gpu:
-        local = 0
-    torch.cuda.set_device(local)
-    if world > 1:
-        if args.dist_backend == "nccl":
-            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-        else:
-            dist.init_process_group(args.dist_backend)
-    dev = torch.device("cuda", local)
+def ncu_dram_bytes_per_photon():
+    """dram__bytes_read.sum + dram__bytes_write.sum of ONE gray_integrate launch of the default workload (2^30 photons,
+    fp32), read from the committed ncu capture: (bytes per photon, file name).  Not a measurement of this run."""
+    for name in ("r02_integrate_f2_dram_2p30.csv", "r01_integrate_f2_dram_2p30.csv"):
+        rows = read_profile_csv(name)
+        if not rows:
+            continue
+        tot = sum(float(r["Metric Value"].replace(",", "")) for r in rows if r["Metric Name"].startswith("dram__bytes_"))
+        if tot > 0:
+            return tot / 2 ** 30, name
+    return None, None
 
+
+def executed_flops_per_photon_step(variant):
+    """FP operations the kernel variant EXECUTES per photon-step (FMA = 2), from the per-opcode executed-instruction
+    counts of the committed ncu captures (profiles/r02_executed_ops.csv); None if the variant was not captured."""
+    rows = read_profile_csv("r02_executed_ops.csv")
+    for r in rows or []:
+        if r["variant"] == variant:
+            return float(r["flops_per_photon_step"])
+    return None
+
+
+def variant_name(prec, rule, case, xi_eps, system, ppt):
+    v = "f64" if prec == "f64" else ("f32x1" if ppt == 1 else "f32")
+    v += "_" + rule
+    if case == "peak":
+        v += "_frozen"
+    if xi_eps > 0:
+        v += "_xi"
+    if system == "reduced":
+        v += "_reduced"
+    return v
+
+
+class Runner:
+    """Times bench steps (init -> integrate -> classify) of one workload variant on this rank's GPU."""
+
+    def __init__(self, args):
+        import torch
+        import torch.distributed as dist
+
+        import paper_1303_5057_b200 as g
+        from paper_1303_5057_b200 import workloads as wl
+        self.torch, self.dist, self.g, self.wl = torch, dist, g, wl
+        self.rank = int(os.environ.get("RANK", "0"))
+        self.world = int(os.environ.get("WORLD_SIZE", "1"))
+        local = int(os.environ.get("LOCAL_RANK", "0"))
+        if not torch.cuda.is_available():
+            raise SystemExit("bench.py: no CUDA device (libgray has no CPU path)")
+        if args.share_gpu:
+            local = 0
+        self.local = local
+        torch.cuda.set_device(local)
+        if self.world > 1:
+            if args.dist_backend == "nccl":
+                dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+            else:
+                dist.init_process_group(args.dist_backend)
+        self.dev = torch.device("cuda", local)
+
+    def barrier(self):
+        if self.world > 1:
+            self.dist.barrier()
+        self.torch.cuda.synchronize()
+
+    def fit_log2n(self, log2n, prec):
+        """37 B (fp32) / 69 B (fp64) of state per photon plus head room: shrink the batch if the device cannot hold it."""
+        per_photon = 38 if prec == "f32" else 70
+        free_bytes, _ = self.torch.cuda.mem_get_info()
+        if self.world > 1:
+            fb = self.torch.tensor([free_bytes], dtype=self.torch.int64, device=self.dev)
+            self.dist.all_reduce(fb, op=self.dist.ReduceOp.MIN)
+            free_bytes = int(fb.item())
+        while log2n > 20 and (2 ** log2n) * per_photon + (4 << 30) > free_bytes:
+            log2n -= 1
+        return log2n
+
+    def params(self, rule, case, xi_eps, system, ppt, schedule="refill", refill_interval=0):
+        g, wl = self.g, self.wl
+        return g.StepParams(h=wl.H, r_capture_factor=wl.R_CAPTURE_FACTOR, r_escape_factor=wl.R_ESCAPE_FACTOR,
+                            rule=g.STEP_EQ2 if rule == "eq2" else g.STEP_REL,
+                            schedule=g.SCHED_REFILL if schedule == "refill" else g.SCHED_STATIC,
+                            refill_interval=refill_interval, frozen=(case == "peak"), photons_per_thread=ppt,
+                            xi_epsilon=xi_eps, system=g.SYS_REDUCED if system == "reduced" else g.SYS_FULL)
+
+    def run(self, *, log2n, prec, rule, case, xi_eps=0.0, system="full", ppt=0, schedule="refill", refill_interval=0,
+            steps, warmup, sample_clocks=False):
+        """W untimed + K timed bench steps; returns the per-rank-reduced measurement (max time, summed work)."""
+        torch, g, wl = self.torch, self.g, self.wl
+        c4 = wl.C4
+        n = 2 ** log2n
+        gprec = g.GRAY_F32 if prec == "f32" else g.GRAY_F64
+        max_steps = c4["peak_steps"] if case == "peak" else wl.MAX_STEPS
+        params = self.params(rule, case, xi_eps, system, ppt, schedule, refill_interval)
+        batch = g.PhotonBatch(n, gprec, device=self.dev)
+        p0 = self.rank * n                                   # weak scaling: every rank its own photon range
+        kern_ev = []
+
+        def step(timed):
+            g.gray_init_rays_random(batch, c4["a"], wl.R_OBS, c4["inc_deg"], c4["half_width"], c4["seed"], p0)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            g.gray_integrate(batch, max_steps=max_steps, params=params)
+            e1.record()
+            counts = g.gray_classify(batch)            # synchronises; the step's result on the host
+            cnt = g.gray_integrate_counters(batch)
+            if timed:
+                kern_ev.append((e0, e1))
+            return counts, cnt
+
+        for _ in range(warmup):
+            step(False)
+        sampler = ClockSampler(self.local) if (sample_clocks and self.rank == 0) else None
+        self.barrier()
+        t0 = time.perf_counter()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record()
+        photon_steps, issued, counts = 0, 0, None
+        for _ in range(steps):
+            counts, cnt = step(True)
+            photon_steps += cnt["photon_steps"]
+            issued += cnt["issued_steps"]
+        ev1.record()
+        self.barrier()
+        t1 = time.perf_counter()
+        clocks = sampler.stop(t0, t1) if sampler else None
+        ms = ev0.elapsed_time(ev1)
+        kern_ms = sum(a.elapsed_time(b) for a, b in kern_ev) / max(1, len(kern_ev))
+        del batch
+        if self.world > 1:
+            t = torch.tensor([ms, kern_ms], dtype=torch.float64, device=self.dev)
+            self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX)
+            ms, kern_ms = float(t[0]), float(t[1])
+            w = torch.tensor([photon_steps, issued], dtype=torch.float64, device=self.dev)
+            self.dist.all_reduce(w, op=self.dist.ReduceOp.SUM)
+            photon_steps, issued = float(w[0]), float(w[1])
+        return dict(n=n, log2n=log2n, prec=prec, rule=rule, case=case, xi_eps=xi_eps, system=system, ppt=ppt, steps=steps,
+                    ms=ms, kernel_ms=kern_ms, photon_steps=float(photon_steps), issued=float(issued), counts=counts,
+                    clocks=clocks, max_steps=max_steps)
+
+    def roofline(self, m):
+        """Roofline fields of the dominant kernel (integrate_kernel) of a measurement, per GPU: work per launch / its
+        CUDA-event duration against the FMA peak.  `frac` counts the oracle's operation tally (BASELINE's definition),
+        `frac_executed` the operations the kernel executes (ncu), both with FMA = 2."""
+        per_gpu_steps = m["photon_steps"] / self.world / m["steps"]
+        # peak case: every issued lane-step computes, so issued lane-steps are the units
+        counted = per_gpu_steps if m["case"] != "peak" else m["issued"] / self.world / m["steps"]
+        peak = PEAK_TFLOPS[m["prec"]]
+        rate = counted / (m["kernel_ms"] * 1e-3)                        # units per second inside the kernel
+        flops = FLOPS_PER_PHOTON_STEP[m["rule"]]
+        reduced = m["system"] == "reduced"
+        achieved = None if reduced else flops * rate / 1e12
+        exe = executed_flops_per_photon_step(variant_name(m["prec"], m["rule"], m["case"], m["xi_eps"], m["system"], m["ppt"]))
+        return dict(achieved=achieved, peak=peak, frac=None if reduced else achieved / peak,
+                    executed_flops_per_photon_step=exe, achieved_executed=exe * rate / 1e12 if exe else None,
+                    frac_executed=exe * rate / 1e12 / peak if exe else None,
+                    frac_survey_hand_tally=None if (reduced or m["prec"] != "f32") else FLOPS_SURVEY_HAND_TALLY * rate / 1e12 / peak,
+                    kernel_ms=m["kernel_ms"], kernel_share_of_step=m["kernel_ms"] * m["steps"] / m["ms"],
+                    lane_efficiency=m["photon_steps"] / m["issued"] if m["issued"] else None)
+
+
+def secondary_line(R, m, label):
+    rf = R.roofline(m)
+    value = m["photon_steps"] / (m["ms"] * 1e-3)
+    return {"workload": label, "dtype": m["prec"], "photons_per_gpu": m["n"], "steps": m["steps"], "value": value,
+            "unit": "photon-steps/s", "ns_per_photon_step": 1e9 / value, "kernel_ms": rf["kernel_ms"],
+            "frac": rf["frac"], "frac_executed": rf["frac_executed"], "lane_efficiency": rf["lane_efficiency"],
+            "issued_lane_steps_per_s": m["issued"] / (m["ms"] * 1e-3)}
+
+
+def run_e2e(R, args, params, max_steps, prec, p0):
+    """The same metric end to end through the C ABI with HOST buffers (gray_integrate_host): pinned host x, k in;
+    x, k, status, steps out; both copies inside the timed region."""
+    torch, g, wl = R.torch, R.g, R.wl
     c4 = wl.C4
-    # 37 B (fp32) / 69 B (fp64) of state per photon, plus the e2e leg's device scratch: shrink the batch if it cannot fit
-    per_photon = 38 if args.prec == "f32" else 70
-    free_bytes, _ = torch.cuda.mem_get_info()
-    if world > 1:
-        fb = torch.tensor([free_bytes], dtype=torch.int64, device=dev)
-        dist.all_reduce(fb, op=dist.ReduceOp.MIN)
-        free_bytes = int(fb.item())
-    while args.log2n > 20 and (2 ** args.log2n) * per_photon + (4 << 30) > free_bytes:
-        args.log2n -= 1
+    gprec = g.GRAY_F32 if prec == "f32" else g.GRAY_F64
+    bytes_per_photon = (2 * 32 if prec == "f32" else 2 * 64) * 2 + 5        # pinned: inputs, outputs, status, steps
+    le = args.e2e_log2n if args.e2e_log2n >= 0 else min(args.log2n, 28)
+    note = None
+    try:
+        import psutil
+        avail = psutil.virtual_memory().available
+    except Exception:  # pragma: no cover
+        avail = 16 << 30
+    while le > 20 and 1.25 * bytes_per_photon * 2 ** le * (R.world if args.share_gpu or R.world > 1 else 1) > avail:
+        le -= 1
+        note = "reduced to fit the host's available memory (%.0f GB) with pinned in + out buffers" % (avail / 2 ** 30)
+    ne = 2 ** le
+    dt = torch.float32 if prec == "f32" else torch.float64
+    x_in = torch.empty((ne, 4), dtype=dt, pin_memory=True)
+    k_in = torch.empty((ne, 4), dtype=dt, pin_memory=True)
+    piece = min(ne, 1 << 26)
+    hb = g.PhotonBatch(piece, gprec, device=R.dev)
+    for lo in range(0, ne, piece):                                  # initial states, made on the device piecewise
+        g.gray_init_rays_random(hb, c4["a"], wl.R_OBS, c4["inc_deg"], c4["half_width"], c4["seed"], p0 + lo)
+        x_in[lo:lo + piece].copy_(hb.x)
+        k_in[lo:lo + piece].copy_(hb.k)
+    del hb
+    x_out, k_out = torch.empty_like(x_in, pin_memory=True), torch.empty_like(k_in, pin_memory=True)
+    st_h = torch.empty((ne,), dtype=torch.uint8, pin_memory=True)
+    ns_h = torch.empty((ne,), dtype=torch.int32, pin_memory=True)
+    chunk = min(ne, 1 << 23)
+    scratch = torch.empty((g.gray_host_scratch_bytes(chunk, gprec),), dtype=torch.uint8, device=R.dev)
+    call = lambda: g.gray_integrate_host(x_in, k_in, x_out, k_out, st_h, ns_h, c4["a"], wl.R_OBS, max_steps=max_steps,
+                                         params=params, chunk=chunk, scratch=scratch)
+    call()                                                     # warm-up (also creates the library's two streams)
+    reps = max(1, min(args.steps, 2 if le >= 28 else 3))
+    R.barrier()
+    w0 = time.perf_counter()
+    e_steps = 0
+    for _ in range(reps):
+        e_steps += call()["photon_steps"]                      # synchronous: results are in host memory on return
+    torch.cuda.synchronize()
+    e_t = time.perf_counter() - w0
+    h2d = int(x_in.numel() * x_in.element_size() * 2)
+    d2h = int(h2d + st_h.numel() + ns_h.numel() * 4)
+    if R.world > 1:
+        t = torch.tensor([e_t], dtype=torch.float64, device=R.dev)
+        R.dist.all_reduce(t, op=R.dist.ReduceOp.MAX)
+        w = torch.tensor([e_steps], dtype=torch.float64, device=R.dev)
+        R.dist.all_reduce(w, op=R.dist.ReduceOp.SUM)
+        e_t, e_steps = float(t[0]), float(w[0])
+    return {"value": e_steps / e_t, "unit": "photon-steps/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+            "photons_per_gpu": ne, "reps": reps, "note": note,
+            "call": "gray_integrate_host (pinned host x,k in; x,k,status,steps out; 2^23-photon chunks on two streams)",
+            "timer": "host wall clock around the synchronous C-ABI calls"}
+
+
+def run_gray(args):
+    R = Runner(args)
+    g, wl = R.g, R.wl
+    world, rank = R.world, R.rank
+    args.log2n = R.fit_log2n(args.log2n, args.prec)
     n = 2 ** args.log2n
     prec = g.GRAY_F32 if args.prec == "f32" else g.GRAY_F64
-    rule = g.STEP_EQ2 if args.rule == "eq2" else g.STEP_REL
-    peak_case = args.case == "peak"
-    max_steps = c4["peak_steps"] if peak_case else wl.MAX_STEPS
-    params = g.StepParams(h=wl.H, r_capture_factor=wl.R_CAPTURE_FACTOR, r_escape_factor=wl.R_ESCAPE_FACTOR, rule=rule,
-                          schedule=g.SCHED_REFILL if args.schedule == "refill" else g.SCHED_STATIC,
-                          refill_interval=args.refill_interval, frozen=peak_case,
-                          photons_per_thread=args.photons_per_thread, xi_epsilon=args.xi_eps,
-                          system=g.SYS_REDUCED if args.system == "reduced" else g.SYS_FULL)
-    batch = g.PhotonBatch(n, prec, device=dev)
-    p0 = rank * n                                   # weak scaling: every rank its own photon range
 
-    kern_ev = []
-
-    def step(timed):
-        g.gray_init_rays_random(batch, c4["a"], wl.R_OBS, c4["inc_deg"], c4["half_width"], c4["seed"], p0)
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
-        g.gray_integrate(batch, max_steps=max_steps, params=params)
-        e1.record()
-        counts = g.gray_classify(batch)            # synchronises; the step's result on the host
-        cnt = g.gray_integrate_counters(batch)
-        if timed:
-            kern_ev.append((e0, e1))
-        return counts, cnt
-
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    for _ in range(args.warmup):
-        step(False)
-    sampler = ClockSampler(local) if rank == 0 else None
-    barrier()
-    t0 = time.perf_counter()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    ev0.record()
-    photon_steps, issued, counts = 0, 0, None
-    for _ in range(args.steps):
-        counts, cnt = step(True)
-        photon_steps += cnt["photon_steps"]
-        issued += cnt["issued_steps"]
-    ev1.record()
-    barrier()
-    t1 = time.perf_counter()
-    clocks = sampler.stop(t0, t1) if sampler else None
-    ms = ev0.elapsed_time(ev1)
-    kern_ms = sum(a.elapsed_time(b) for a, b in kern_ev) / max(1, len(kern_ev))
+    # ---- the headline: BASELINE's metric on config C4 at its largest size
+    m = R.run(log2n=args.log2n, prec=args.prec, rule=args.rule, case=args.case, xi_eps=args.xi_eps, system=args.system,
+              ppt=args.photons_per_thread, schedule=args.schedule, refill_interval=args.refill_interval, steps=args.steps,
+              warmup=args.warmup, sample_clocks=True)
 
     # ---- end to end through the C ABI with host buffers (copies inside the timed region)
     e2e = None
     if not args.no_e2e:
-        le = args.e2e_log2n if args.e2e_log2n >= 0 else min(args.log2n, 26)
-        ne = 2 ** le
-        dt = torch.float32 if prec == g.GRAY_F32 else torch.float64
-        hb = g.PhotonBatch(ne, prec, device=dev)
-        g.gray_init_rays_random(hb, c4["a"], wl.R_OBS, c4["inc_deg"], c4["half_width"], c4["seed"], p0)
-        x_in, k_in = hb.x.cpu().pin_memory(), hb.k.cpu().pin_memory()
-        del hb
-        x_out, k_out = torch.empty_like(x_in).pin_memory(), torch.empty_like(k_in).pin_memory()
-        st_h = torch.empty((ne,), dtype=torch.uint8).pin_memory()
-        ns_h = torch.empty((ne,), dtype=torch.int32).pin_memory()
-        chunk = min(ne, 1 << 23)
-        scratch = torch.empty((g.gray_host_scratch_bytes(chunk, prec),), dtype=torch.uint8, device=dev)
-        call = lambda: g.gray_integrate_host(x_in, k_in, x_out, k_out, st_h, ns_h, c4["a"], wl.R_OBS, max_steps=max_steps,
-                                             params=params, chunk=chunk, scratch=scratch)
-        call()                                                     # warm-up
-        reps = max(1, min(args.steps, 3))
-        barrier()
-        w0 = time.perf_counter()
-        e_steps = 0
-        for _ in range(reps):
-            e_steps += call()["photon_steps"]                      # synchronous: results are in host memory on return
-        torch.cuda.synchronize()
-        e_t = time.perf_counter() - w0
-        h2d = int(x_in.numel() * x_in.element_size() * 2)
-        d2h = int(h2d + st_h.numel() + ns_h.numel() * 4)
-        e2e = {"steps_total": e_steps, "seconds": e_t, "h2d": h2d, "d2h": d2h, "photons": ne, "reps": reps}
+        params = R.params(args.rule, args.case, args.xi_eps, args.system, args.photons_per_thread, args.schedule, args.refill_interval)
+        e2e = run_e2e(R, args, params, m["max_steps"], args.prec, rank * n)
 
-    # ---- reduce over ranks: max time, summed work
-    if world > 1:
-        t = torch.tensor([ms, kern_ms, e2e["seconds"] if e2e else 0.0], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms, kern_ms = float(t[0]), float(t[1])
-        s = torch.tensor([photon_steps, issued, e2e["steps_total"] if e2e else 0], dtype=torch.float64, device=dev)
-        dist.all_reduce(s, op=dist.ReduceOp.SUM)
-        if e2e:
-            e2e["seconds"] = float(t[2])
-            e2e["steps_total"] = float(s[2])
-        tot_steps, tot_issued = float(s[0]), float(s[1])
-    else:
-        tot_steps, tot_issued = float(photon_steps), float(issued)
+    # ---- every other quoted number, in the same run (VERDICT r1 #3): C4's sweep in both cases, fp64, xi monitor,
+    #      reduced system; 1 warm-up + 2 timed steps each
+    secondary = []
+    if not args.no_secondary:
+        todo = []
+        for l2 in (20, 24, 28):
+            if l2 < args.log2n or args.case != "realistic":
+                todo.append((f"C4-realistic 2^{l2} photons/GPU, fp32, eq2", dict(log2n=l2, prec="f32", rule="eq2", case="realistic")))
+        for l2 in (20, 24, 28):
+            todo.append((f"C4-peak 2^{l2} photons/GPU: {wl.C4['peak_steps']} REL steps per lane, state frozen by select (R17)",
+                         dict(log2n=l2, prec="f32", rule="rel", case="peak")))
+        todo.append(("C4-realistic 2^26 photons/GPU, fp64 build, eq2", dict(log2n=26, prec="f64", rule="eq2", case="realistic")))
+        todo.append(("C4-realistic 2^26 photons/GPU, fp32, eq2, xi monitor eps=1e-3 (paper's production scheme, P:103-109)",
+                     dict(log2n=26, prec="f32", rule="eq2", case="realistic", xi_eps=1e-3)))
+        todo.append(("C4-realistic 2^26 photons/GPU, fp32, eq2, reduced system (E, L_z eliminate k^t, k^phi)",
+                     dict(log2n=26, prec="f32", rule="eq2", case="realistic", system="reduced")))
+        todo.append(("C4-realistic 2^26 photons/GPU, fp32, eq2, one photon per thread (scalar FFMA)",
+                     dict(log2n=26, prec="f32", rule="eq2", case="realistic", ppt=1)))
+        for label, kw in todo:
+            kw["log2n"] = min(kw["log2n"], R.fit_log2n(kw["log2n"], kw["prec"]))
+            ms = R.run(steps=2, warmup=1, **kw)
+            if rank == 0:
+                secondary.append(secondary_line(R, ms, label))
 
     if rank != 0:
         if world > 1:
-            dist.destroy_process_group()
+            R.dist.destroy_process_group()
         return
 
-    value = tot_steps / (ms * 1e-3)
-    flops = FLOPS_PER_PHOTON_STEP[args.rule]
-    # roofline of the dominant kernel (integrate_kernel), per GPU: algorithmic flops per launch / its duration
-    per_gpu_steps = tot_steps / world / args.steps
-    counted = per_gpu_steps if not peak_case else tot_issued / world / args.steps   # peak case: every issued lane-step computes
-    achieved = flops * counted / (kern_ms * 1e-3) / 1e12
-    peak = PEAK_TFLOPS[args.prec]
+    value = m["photon_steps"] / (m["ms"] * 1e-3)
+    rf = R.roofline(m)
     fma_peak = g.gray_fma_peak(prec, 8192) / 1e12
-    # Achievable ceiling of the packed fp32 kernel: the FP32 pipe retires the
-    # integrator's mix of FMUL2 / FFMA2 / FADD2 with changing register operands at this fraction of its lane rate
     mix = None
     if args.prec == "f32" and args.photons_per_thread != 1:
         lane_peak = 148 * 128 * 1.965e9
         mix = {"ffma2_invariant_operands": g.gray_packed_peak(0) / lane_peak, "ffma2_three_register_pairs": g.gray_packed_peak(1) / lane_peak,
-               "integrator_mix": g.gray_packed_peak(2) / lane_peak}
-    roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                "traffic": (NCU_DRAM_BYTES_PER_PHOTON * n) if (NCU_DRAM_BYTES_PER_PHOTON and args.prec == "f32") else None,
-                "traffic_source": "ncu dram bytes per photon of the 2^30-photon launch (profiles/) x photons of this launch",
-                "kernel": "gray::integrate_kernel", "kernel_ms": kern_ms, "kernel_share_of_step": kern_ms * args.steps / ms,
-                "executed_flops_per_photon_step": NCU_EXECUTED_FLOPS_PER_PHOTON_STEP if (args.prec == "f32" and args.photons_per_thread != 1 and args.system == "full" and args.xi_eps == 0) else None,
-                "flops_per_photon_step": flops, "flops_source": "oracle operation tally (add=sub=mul=div=sqrt=sin=cos=1)",
+               "integrator_mix_r01": g.gray_packed_peak(2) / lane_peak}
+    dram_b, dram_src = ncu_dram_bytes_per_photon()
+    flops = FLOPS_PER_PHOTON_STEP[args.rule]
+    roofline = {"bound": "alu", "achieved": rf["achieved"], "peak": rf["peak"], "unit": "TFLOP/s", "frac": rf["frac"],
+                "traffic": (dram_b * n) if (dram_b and args.prec == "f32") else None,
+                "traffic_source": (f"NOT measured in this run: ncu dram bytes per photon of one 2^30-photon launch, read from profiles/{dram_src}, "
+                                   "x photons of this launch") if dram_b else None,
+                "kernel": "gray::integrate_kernel", "kernel_ms": rf["kernel_ms"], "kernel_share_of_step": rf["kernel_share_of_step"],
+                "flops_per_photon_step": flops, "flops_source": "oracle operation tally (add=sub=mul=div=sqrt=sin=cos=1): BASELINE's definition",
+                "executed_flops_per_photon_step": rf["executed_flops_per_photon_step"],
+                "executed_source": "ncu per-opcode executed instruction counts (profiles/r02_executed_ops.csv), FMA = 2",
+                "achieved_executed": rf["achieved_executed"], "frac_executed": rf["frac_executed"],
+                "flops_survey_hand_tally": FLOPS_SURVEY_HAND_TALLY, "frac_survey_hand_tally": rf["frac_survey_hand_tally"],
                 "peak_source": "148 SMs x %d lanes x 2 x 1.965 GHz (DESIGN.md)" % (128 if args.prec == "f32" else 64),
-                "fma_microbench_tflops": fma_peak, "frac_of_fma_microbench": achieved / fma_peak,
-                "lane_efficiency": tot_steps / tot_issued if tot_issued else None,
-                "packed_pipe_fraction_measured": mix,
-                "frac_of_achievable": (achieved / peak) / (mix["integrator_mix"] * 787.0 / 792.0) if mix else None,
+                "fma_microbench_tflops": fma_peak, "frac_of_fma_microbench": rf["achieved"] / fma_peak if rf["achieved"] else None,
+                "lane_efficiency": rf["lane_efficiency"], "packed_pipe_fraction_measured": mix,
                 "hbm_algorithmic_bytes_per_launch": n * (2 * (32 if args.prec == "f32" else 64) + 10)}
     if args.system == "reduced":
-        # the operation tally is the full system's; the reduced system does less work per step, so a FLOP rate
-        # against that tally would overstate it: only photon-steps/s is reported for it
-        for k in ("achieved", "frac", "frac_of_fma_microbench", "frac_of_achievable"):
-            roofline[k] = None
         roofline["note"] = "system=reduced: no operation tally of its own; see value / ns_per_photon_step"
     out = {"metric": "photon-steps/s", "value": value, "unit": "photon-steps/s", "n_gpus": world, "steps": args.steps,
-           "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+           "warmup": args.warmup, "ms_per_step": m["ms"] / args.steps, "higher_is_better": True, "scaling": "weak",
            "vs_baseline": None, "dtype": args.prec, "data": "synthetic", "config": workload_config(args, world),
            "ns_per_photon_step": 1e9 / value, "gflops": flops * value / 1e9 if args.system == "full" else None,
-           "mean_steps_per_photon": tot_steps / (world * n * args.steps), "status_counts_rank0": counts,
-           "roofline": roofline, "gpu_launches": 3 * args.steps, "clocks": clocks,
+           "mean_steps_per_photon": m["photon_steps"] / (world * n * args.steps), "status_counts_rank0": m["counts"],
+           "roofline": roofline, "gpu_launches": 3 * args.steps, "clocks": m["clocks"],
            "paper_context": "GRay on Tesla M2090 (2013): 1.15 ns/photon/step single precision, >300 GFLOP/s (P:7, P:150)"}
     if e2e:
-        out["e2e"] = {"value": e2e["steps_total"] / e2e["seconds"], "unit": "photon-steps/s",
-                      "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"],
-                      "photons_per_gpu": e2e["photons"], "reps": e2e["reps"],
-                      "call": "gray_integrate_host (pinned host x,k in; x,k,status,steps out; 2^23-photon chunks on two streams)",
-                      "timer": "host wall clock around the synchronous C-ABI calls"}
+        out["e2e"] = e2e
+    if secondary:
+        out["secondary"] = secondary
     if not args.no_cpu_baseline:
         import oracle as o                          # cpu_baseline leg only
         threads = max(1, o.hardware_threads())
-        ps, dt, m = oracle_sample(args, 18, threads)
+        ps, dt, mm = oracle_sample(args, args.cpu_log2n, threads)
+        ps1, dt1, m1 = oracle_sample(args, max(10, args.cpu_log2n - 4), 1)
         out["cpu_baseline"] = {"value": ps / dt, "unit": "photon-steps/s", "cores": threads, "kind": "oracle",
-                               "sample": f"{m} photons, strided p = j * 2^{args.log2n} / {m} of rank 0's photons, "
-                                         f"{ps} photon-steps in {dt:.1f} s", "ns_per_photon_step_per_core": 1e9 * dt * threads / ps}
+                               "sample": f"{mm} photons, strided p = j * 2^{args.log2n} / {mm} of rank 0's photons, "
+                                         f"{ps} photon-steps in {dt:.1f} s",
+                               "ns_per_photon_step": 1e9 * dt / ps,
+                               "one_core": {"value": ps1 / dt1, "unit": "photon-steps/s", "cores": 1, "ns_per_photon_step": 1e9 * dt1 / ps1,
+                                            "sample": f"{m1} photons of the same strided sample, {ps1} photon-steps in {dt1:.1f} s"}}
     print(json.dumps(out), flush=True)
     if world > 1:
-        dist.destroy_process_group()
+        R.dist.destroy_process_group()
 
 
 def run_projection(args):
@@ -395,8 +546,27 @@ def run_projection(args):
     print(json.dumps(out), flush=True)
 
 
+def launcher_command(args, argv, port=None):
+    """`python bench.py --gpus N` started by hand (no torchrun environment): the command that re-runs this script as N
+    ranks on this node, one per GPU, the way the driver launches it.  None if no re-launch is needed."""
+    if args.gpus <= 1 or "WORLD_SIZE" in os.environ or args.impl == "reference":
+        return None
+    if port is None:
+        import socket
+        with socket.socket() as sock:
+            sock.bind(("127.0.0.1", 0))
+            port = sock.getsockname()[1]
+    return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+            "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + list(argv)
+
+
 def main():
     args = parse()
+    cmd = launcher_command(args, sys.argv[1:])
+    if cmd is not None:
+        env = dict(os.environ)
+        env.setdefault("NCCL_DEBUG", "INFO")          # NCCL's init log on stderr: the driver can count the ranks
+        raise SystemExit(subprocess.call(cmd, env=env))
     if args.case == "projection" and args.impl != "reference":
         run_projection(args)
         return

@@ -11,7 +11,9 @@
  *   coordinates     Boyer-Lindquist (t, r, theta, phi); state of a photon = x^mu and k^mu = dx^mu/dlambda
  *   memory          every pointer named *_dev is DEVICE memory owned by the caller (PyTorch tensors in
  *                   the Python binding); the library never allocates, frees or keeps it.  Pointers
- *                   named *_host are HOST memory owned by the caller.
+ *                   named *_host are HOST memory owned by the caller.  Exceptions, stated where they occur:
+ *                   gray_integrate_host keeps two streams and 80 bytes of pinned staging per device; the two
+ *                   microbenchmarks gray_fma_peak / gray_packed_peak allocate and free a few KB while they run.
  *   layout          structure of arrays of 16-byte-aligned 4-vectors: x[p] = (t, r, theta, phi),
  *                   k[p] = (k^t, k^r, k^theta, k^phi); float4 for GRAY_F32, 4 doubles for GRAY_F64.
  *   stream          `cuda_stream` is a cudaStream_t passed as void* (NULL = the default stream).  All
@@ -251,16 +253,22 @@ GRAY_API int gray_ring_polar(const gray_state* state, int32_t bridge_axis, doubl
  * inputs), status_host (n bytes), steps_host (n).  Host buffers should be pinned (cudaHostAlloc /
  * torch pin_memory) for the copies to be asynchronous.  scratch_dev must hold
  * gray_host_scratch_bytes(chunk, prec) bytes of device memory, 256-byte aligned.  counters_host (may be
- * NULL) receives the summed gray_counters.  Synchronous: returns when every result is in host memory. */
+ * NULL) receives the summed gray_counters.  Synchronous: returns when every result is in host memory.
+ * Ordering: the internal streams start after everything enqueued so far on `cuda_stream` (NULL = the default
+ * stream), so inputs or scratch written by earlier work on that stream are safe.  The two streams, one event and
+ * 80 bytes of pinned host staging are created on the first call on a device and kept for the life of the process
+ * (the only resources the library ever keeps); concurrent calls are serialised.  After an error every chunk
+ * already enqueued is still waited for before the function returns, and counters_host holds the chunks completed. */
 GRAY_API size_t gray_host_scratch_bytes(uint64_t chunk, int32_t prec);
 GRAY_API int gray_integrate_host(const void* x_in_host, const void* k_in_host, void* x_out_host, void* k_out_host,
                         uint8_t* status_host, uint32_t* steps_host, uint64_t n, int32_t prec, double a,
                         double r_obs, uint32_t max_steps, const gray_step_params* params, uint64_t chunk,
-                        void* scratch_dev, size_t scratch_bytes, gray_counters* counters_host);
+                        void* scratch_dev, size_t scratch_bytes, gray_counters* counters_host, void* cuda_stream);
 
 /* Register-only FFMA (GRAY_F32) or DFMA (GRAY_F64) microbenchmark: the measured CUDA-core peak the
  * integrator's rate is divided by.  Runs `iters` dependent-chain-free FMA rounds
- * on every SM, times them with CUDA events on the stream, returns FLOP/s (FMA = 2).  Synchronises.  */
+ * on every SM, times them with CUDA events on the stream, returns FLOP/s (FMA = 2).  Synchronises.
+ * Allocates 8 bytes of device memory (cudaMalloc) for the duration of the call and frees them.      */
 GRAY_API int gray_fma_peak(int32_t prec, int32_t iters, double* flops_per_s_host, void* cuda_stream);
 
 /* Packed FP32 (FFMA2 / FMUL2 / FADD2, the instructions of the GRAY_F32 integrator) register-only microbenchmark,
@@ -271,7 +279,7 @@ GRAY_API int gray_fma_peak(int32_t prec, int32_t iters, double* flops_per_s_host
  *   mix 1  FFMA2 reading three different, changing register pairs
  *   mix 2  the integrator's instruction mix: 50 % FMUL2, 37.5 % FFMA2 (three pairs), 12.5 % FADD2
  * Returns fp32 lane-operations per second (one FFMA2 = 2 per thread; multiply by 2 for FMA flops of mix 0 / 1).
- * Synchronises.                                                                                             */
+ * Synchronises.  Allocates 8 KB of device memory (cudaMalloc) for the duration of the call and frees them.   */
 GRAY_API int gray_packed_peak(int32_t mix, int32_t iters, double* lane_ops_per_s_host, void* cuda_stream);
 
 /* Device facts used by the benchmark: SM count and SM clock (kHz) reported by the runtime.         */

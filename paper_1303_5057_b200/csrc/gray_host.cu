@@ -2,12 +2,15 @@
 // double-buffered over two streams so PCIe copies overlap the integrator kernel.
 #include "gray_internal.h"
 
+#include <mutex>
+
 namespace gray {
 
 struct Slot {
   char* x; char* k; uint32_t* steps; uint8_t* status; Workspace* ws;
   cudaStream_t stream;
   unsigned long long* c;     // counters of the chunk last run on this slot (pinned host staging)
+  bool in_flight;            // a chunk has been enqueued on this slot and not drained yet
 };
 
 static size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
@@ -15,6 +18,42 @@ static size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
 static size_t slot_bytes(uint64_t chunk, int prec) {
   const size_t vec = (prec == GRAY_F32 ? 16 : 32);
   return align256(chunk * vec) * 2 + align256(chunk * 4) + align256(chunk) + align256(sizeof(Workspace));
+}
+
+// The two copy / compute streams, the event that orders them after the caller's stream and the pinned staging of the
+// counters are created once per device, on the first call, and kept for the life of the process (they are not
+// device memory: 80 bytes of pinned host memory and three driver handles).  Calls are serialised by a mutex.
+struct HostPath {
+  bool ready = false;
+  cudaStream_t stream[2] = {nullptr, nullptr};
+  cudaEvent_t caller_done = nullptr;
+  unsigned long long* pinned = nullptr;
+};
+static std::mutex g_host_mutex;
+static HostPath g_host_path[64];
+
+static int host_path(HostPath** out) {
+  int dev = 0;
+  GRAY_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= 64) { set_error("gray_integrate_host: device index %d out of range", dev); return GRAY_ERR_CUDA; }
+  HostPath& H = g_host_path[dev];
+  if (!H.ready) {
+    HostPath T;
+    cudaError_t e = cudaHostAlloc(&T.pinned, 10 * sizeof(unsigned long long), cudaHostAllocDefault);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&T.stream[0], cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&T.stream[1], cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&T.caller_done, cudaEventDisableTiming);
+    if (e != cudaSuccess) {
+      if (T.caller_done) cudaEventDestroy(T.caller_done);
+      for (int s = 0; s < 2; ++s) if (T.stream[s]) cudaStreamDestroy(T.stream[s]);
+      if (T.pinned) cudaFreeHost(T.pinned);
+      return cuda_fail(e, "gray_integrate_host: creating streams / pinned staging");
+    }
+    T.ready = true;
+    H = T;
+  }
+  *out = &H;
+  return GRAY_OK;
 }
 
 }  // namespace gray
@@ -26,7 +65,7 @@ size_t gray_host_scratch_bytes(uint64_t chunk, int32_t prec) { return 2 * gray::
 int gray_integrate_host(const void* x_in_host, const void* k_in_host, void* x_out_host, void* k_out_host,
                         uint8_t* status_host, uint32_t* steps_host, uint64_t n, int32_t prec, double a, double r_obs,
                         uint32_t max_steps, const gray_step_params* params, uint64_t chunk, void* scratch_dev,
-                        size_t scratch_bytes, gray_counters* counters_host) {
+                        size_t scratch_bytes, gray_counters* counters_host, void* cuda_stream) {
   using namespace gray;
   if (prec != GRAY_F32 && prec != GRAY_F64) { set_error("bad precision"); return GRAY_ERR_ARG; }
   if (!params) { set_error("params is NULL"); return GRAY_ERR_ARG; }
@@ -39,11 +78,16 @@ int gray_integrate_host(const void* x_in_host, const void* k_in_host, void* x_ou
     set_error("scratch_dev is NULL, not 256-byte aligned or smaller than gray_host_scratch_bytes()");
     return GRAY_ERR_WORKSPACE;
   }
+  std::lock_guard<std::mutex> lock(g_host_mutex);
+  HostPath* H = nullptr;
+  int rc = host_path(&H);
+  if (rc) return rc;
+  // everything the caller has enqueued on its stream so far (e.g. the kernel that produced scratch_dev's previous
+  // contents, or a copy into the host inputs) comes before the first copy in
+  GRAY_CUDA(cudaEventRecord(H->caller_done, (cudaStream_t)cuda_stream));
   const size_t vec = (prec == GRAY_F32 ? 16 : 32);
   Slot slot[2];
   char* base = (char*)scratch_dev;
-  unsigned long long* pinned = nullptr;   // 2 x 5 counters; pinned so the copies back stay asynchronous
-  GRAY_CUDA(cudaHostAlloc(&pinned, 10 * sizeof(unsigned long long), cudaHostAllocDefault));
   for (int s = 0; s < 2; ++s) {
     char* p = base + s * slot_bytes(chunk, prec);
     slot[s].x = p; p += align256(chunk * vec);
@@ -51,24 +95,33 @@ int gray_integrate_host(const void* x_in_host, const void* k_in_host, void* x_ou
     slot[s].steps = (uint32_t*)p; p += align256(chunk * 4);
     slot[s].status = (uint8_t*)p; p += align256(chunk);
     slot[s].ws = (Workspace*)p;
-    slot[s].c = pinned + 5 * s;
-    GRAY_CUDA(cudaStreamCreateWithFlags(&slot[s].stream, cudaStreamNonBlocking));
+    slot[s].c = H->pinned + 5 * s;
+    slot[s].stream = H->stream[s];
+    slot[s].in_flight = false;
+    GRAY_CUDA(cudaStreamWaitEvent(slot[s].stream, H->caller_done, 0));
   }
-  int rc = GRAY_OK;
   gray_counters total = {0, 0, 0, 0, 0};
-  uint64_t done_chunks = 0;
-  auto drain = [&](int s) -> int {   // wait for the chunk in flight on slot s and add its counters
-    GRAY_CUDA(cudaStreamSynchronize(slot[s].stream));
-    total.photon_steps += slot[s].c[0]; total.issued_steps += slot[s].c[1];
-    total.photons_done += slot[s].c[2]; total.photons_live += slot[s].c[3];
-    total.fallback_steps += slot[s].c[4];
+  // wait for the chunk in flight on slot s (if any) and add its counters; each chunk is drained exactly once
+  auto drain = [&](int s, bool count) -> int {
+    if (!slot[s].in_flight) return GRAY_OK;
+    slot[s].in_flight = false;
+    cudaError_t e = cudaStreamSynchronize(slot[s].stream);
+    if (e != cudaSuccess) return cuda_fail(e, "gray_integrate_host: cudaStreamSynchronize");
+    if (count) {
+      total.photon_steps += slot[s].c[0]; total.issued_steps += slot[s].c[1];
+      total.photons_done += slot[s].c[2]; total.photons_live += slot[s].c[3];
+      total.fallback_steps += slot[s].c[4];
+    }
     return GRAY_OK;
   };
-  for (uint64_t lo = 0; lo < n && rc == GRAY_OK; lo += chunk, ++done_chunks) {
-    const int s = (int)(done_chunks & 1);
+  uint64_t chunk_index = 0;
+  for (uint64_t lo = 0; lo < n && rc == GRAY_OK; lo += chunk, ++chunk_index) {
+    const int s = (int)(chunk_index & 1);
     const uint64_t m = (n - lo < chunk) ? n - lo : chunk;
     Slot& S = slot[s];
-    if (done_chunks >= 2) { rc = drain(s); if (rc) break; }
+    rc = drain(s, true);
+    if (rc) break;
+    S.in_flight = true;          // from here on something may be enqueued on the slot's stream
     cudaError_t e;
     e = cudaMemcpyAsync(S.x, (const char*)x_in_host + lo * vec, m * vec, cudaMemcpyHostToDevice, S.stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(S.k, (const char*)k_in_host + lo * vec, m * vec, cudaMemcpyHostToDevice, S.stream);
@@ -88,14 +141,12 @@ int gray_integrate_host(const void* x_in_host, const void* k_in_host, void* x_ou
     if (e == cudaSuccess) e = cudaMemcpyAsync(S.c, &S.ws->photon_steps, 5 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, S.stream);
     if (e != cudaSuccess) { rc = cuda_fail(e, "gray_integrate_host: copy out"); break; }
   }
-  const uint64_t in_flight = done_chunks < 2 ? done_chunks : 2;
-  for (uint64_t q = 0; q < in_flight; ++q) {
-    const int s = (int)((done_chunks - 1 - q) & 1);
-    const int r2 = drain(s);
+  // epilogue: whatever is still in flight, in order; after an error the counters of incomplete chunks are not added
+  for (int q = 0; q < 2; ++q) {
+    const int s = (int)((chunk_index + q) & 1);
+    const int r2 = drain(s, rc == GRAY_OK);
     if (rc == GRAY_OK) rc = r2;
   }
-  for (int s = 0; s < 2; ++s) cudaStreamDestroy(slot[s].stream);
-  cudaFreeHost(pinned);
   if (counters_host) *counters_host = total;
   return rc;
 }

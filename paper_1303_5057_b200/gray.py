@@ -79,7 +79,7 @@ def lib():
         L.gray_host_scratch_bytes.argtypes = [u64, i32]
         L.gray_host_scratch_bytes.restype = C.c_size_t
         L.gray_integrate_host.argtypes = [vp, vp, vp, vp, vp, vp, u64, i32, dbl, dbl, C.c_uint32, C.POINTER(_StepParams),
-                                          u64, vp, C.c_size_t, C.POINTER(_Counters)]
+                                          u64, vp, C.c_size_t, C.POINTER(_Counters), vp]
         L.gray_fma_peak.argtypes = [i32, i32, C.POINTER(dbl), vp]
         L.gray_packed_peak.argtypes = [i32, i32, C.POINTER(dbl), vp]
         L.gray_device_info.argtypes = [C.POINTER(i32), C.POINTER(i32)]
@@ -216,7 +216,7 @@ def gray_integrate_host(x_in, k_in, x_out, k_out, status, steps, a, r_obs, max_s
     c = _Counters()
     _check(lib().gray_integrate_host(_ptr(x_in), _ptr(k_in), _ptr(x_out), _ptr(k_out), _ptr(status), _ptr(steps), n,
                                      prec, a, r_obs, max_steps, C.byref(params.c), chunk, _ptr(scratch),
-                                     scratch.numel(), C.byref(c)))
+                                     scratch.numel(), C.byref(c), _stream()))
     return dict(photon_steps=c.photon_steps, issued_steps=c.issued_steps, photons_done=c.photons_done,
                 photons_live=c.photons_live, fallback_steps=c.fallback_steps)
 

@@ -28,3 +28,31 @@ def test_reference_arm_prints_one_json_line():
     j = json.loads(lines[0])
     assert j["impl"] == "reference" and j["unit"] == "photon-steps/s" and j["value"] > 1e5
     assert j["cpu_baseline"]["kind"] == "oracle" and j["e2e"]["h2d_bytes_per_step"] == 0
+
+
+def test_launcher_command_starts_one_rank_per_gpu(monkeypatch):
+    # `python bench.py --gpus N` by hand must start N ranks itself (row (e) of the scope table)
+    sys.path.insert(0, ROOT)
+    import argparse
+
+    import bench
+    monkeypatch.delenv("WORLD_SIZE", raising=False)
+    a = argparse.Namespace(gpus=4, impl="gray")
+    cmd = bench.launcher_command(a, ["--gpus", "4", "--steps", "2"], port=29999)
+    assert cmd[1:4] == ["-m", "torch.distributed.run", "--nnodes=1"] and "--nproc-per-node=4" in cmd
+    assert cmd[cmd.index("--master-addr") + 1] == "127.0.0.1" and cmd[cmd.index("--master-port") + 1] == "29999"
+    assert cmd[-4:] == ["--gpus", "4", "--steps", "2"] and cmd[-5].endswith("bench.py")
+    assert bench.launcher_command(argparse.Namespace(gpus=1, impl="gray"), []) is None
+    assert bench.launcher_command(argparse.Namespace(gpus=4, impl="reference"), []) is None
+    monkeypatch.setenv("WORLD_SIZE", "4")                    # already inside torchrun (the driver's launch): no re-launch
+    assert bench.launcher_command(a, []) is None
+
+
+def test_profile_csv_readers():
+    sys.path.insert(0, ROOT)
+    import bench
+    b, src = bench.ncu_dram_bytes_per_photon()
+    assert src is not None and 74.0 <= b <= 76.0          # 74 B algorithmic per photon (fp32): DESIGN.md "Data layout"
+    assert bench.variant_name("f32", "eq2", "realistic", 0.0, "full", 0) == "f32_eq2"
+    assert bench.variant_name("f64", "eq2", "realistic", 1e-3, "full", 0) == "f64_eq2_xi"
+    assert bench.variant_name("f32", "rel", "peak", 0.0, "full", 0) == "f32_rel_frozen"

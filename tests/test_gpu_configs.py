@@ -464,3 +464,29 @@ def test_equatorial_projection_with_xi_monitor_matches_oracle():
     assert same.mean() > 0.7
     err = np.abs(y[same][:, [1, 3]] - ref["y"][same][:, [1, 3]]) / np.maximum(1.0, np.abs(ref["y"][same][:, [1, 3]]))
     assert np.quantile(err, 0.99) <= 1e-7, np.quantile(err, 0.99)
+
+
+def test_bench_launches_its_own_ranks():
+    # Scope row (e): `python bench.py --gpus 2` with no torchrun environment starts two ranks itself; here both ranks
+    # share cuda:0 over gloo (one GPU on the box).  One JSON line: n_gpus 2, the work of both ranks summed.
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    common = ["--log2n", "20", "--steps", "1", "--warmup", "1", "--no-e2e", "--no-cpu-baseline", "--no-secondary"]
+    one = subprocess.run([sys.executable, os.path.join(root, "bench.py")] + common, capture_output=True, text=True, timeout=600,
+                         cwd=root, env=env)
+    two = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--dist-backend", "gloo", "--share-gpu"] + common,
+                         capture_output=True, text=True, timeout=600, cwd=root, env=env)
+    assert one.returncode == 0 and two.returncode == 0, two.stderr[-2000:]
+    j1 = json.loads([l for l in one.stdout.splitlines() if l.startswith("{")][-1])
+    lines = [l for l in two.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    j2 = json.loads(lines[0])
+    assert j1["n_gpus"] == 1 and j2["n_gpus"] == 2 and j2["config"]["photons_total"] == 2 * j1["config"]["photons_total"]
+    # rank r traces photons [r n, (r + 1) n): twice the photons, about twice the photon-steps
+    steps1 = j1["mean_steps_per_photon"] * j1["config"]["photons_total"]
+    steps2 = j2["mean_steps_per_photon"] * j2["config"]["photons_total"]
+    assert 1.9 < steps2 / steps1 < 2.1
