@@ -273,8 +273,7 @@ GRAY_DEV void geodesic_accel(const Consts<V>& K, V d, V s, V c, V kt, V kr, V kh
   out[1] = vfma(krkr, G, ACC ? vfma(iS, J2, add[1]) : vmul(iS, J2));
   // dk^theta
   const V w = vfma(K.na, u, Sgk);                           // rho k^phi - a k^t  (= Sigma k^phi - a u)
-  const V a2z1 = vfma(K.na2, vmul(krD, kr), vmul(K.a2, kh2));
-  const V z2 = vfma(Dl, kp2, a2z1);
+  const V z2 = vfma(K.a2, vfma(vneg(krD), kr, kh2), vmul(Dl, kp2));     // Delta (k^phi)^2 + a^2 ((k^th)^2 - (k^r)^2 / Delta)
   const V z3 = vfma(vmul(r, vmul(w, w)), vneg(tiS2), z2);
   const V z5 = vfma(K.m2, vmul(vmul(r, kr), kh), vmul(sc, z3));
   out[2] = ACC ? vfma(iS, z5, add[2]) : vmul(iS, z5);
@@ -290,8 +289,8 @@ GRAY_DEV V step_size(const Consts<V>& K, V d, V kr, V kh, V kp) {
   if (RULE == 0) return nhr;
   const V akr = vabs(kr);
   const V den = vfma(r, vadd(vabs(kh), vabs(kp)), akr);       // r (|k^r|/r + |k^th| + |k^phi|)
-  const V d1 = vmul(nhr, vrcp(den));
-  const V d2 = vmul(vmul(K.nhalf, d), vrcp(akr));
+  const V d1 = vmul(nhr, vrcp_step(den));
+  const V d2 = vmul(vmul(K.nhalf, d), vrcp_step(akr));
   return vmax(d1, d2);
 }
 
@@ -512,8 +511,7 @@ GRAY_DEV void geodesic_accel_reduced(const Consts<V>& K, V d, V s, V c, V kr, V 
   const V J2 = vfma(K.twoa2, vmul(tk, kr), vmul(Dl, Bp));
   out[0] = vfma(krkr, G, ACC ? vfma(iS, J2, add[0]) : vmul(iS, J2));
   // dk^theta
-  const V a2z1 = vfma(K.na2, vmul(krD, kr), vmul(K.a2, kh2));
-  const V z2 = vfma(Dl, kp2, a2z1);
+  const V z2 = vfma(K.a2, vfma(vneg(krD), kr, kh2), vmul(Dl, kp2));     // Delta (k^phi)^2 + a^2 ((k^th)^2 - (k^r)^2 / Delta)
   const V z3 = vfma(vmul(r, vmul(w, w)), vneg(tiS2), z2);
   const V z5 = vfma(K.m2, vmul(vmul(r, kr), kh), vmul(sc, z3));
   out[1] = ACC ? vfma(iS, z5, add[1]) : vmul(iS, z5);

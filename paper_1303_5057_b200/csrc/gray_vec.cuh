@@ -109,17 +109,26 @@ GRAY_DEV float srcp(float x) {
   return y;
 }
 GRAY_DEV float vrcp(float x) { return srcp(x); }
-// double: MUFU.RCP64H seed (rcp.approx.ftz.f64, ~2^-20) and two Newton iterations in FMAs: relative error
-// ~1e-16 (not correctly rounded, like the float build's), no special-case branch; 4 FP64 operations.
+// double: MUFU.RCP64H seed y0 (rcp.approx.ftz.f64, relative error e ~ 2^-20) refined to third order in FMAs,
+// y = y0 (1 + e + e^2) with e = 1 - x y0: relative error e^3 ~ 1e-18, i.e. the rounding of the last FMA (not correctly
+// rounded, like the float build's); 3 FP64 operations, no special-case branch.
 GRAY_DEV double vrcp(double x) {
   double y;
   asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-  double e = __fma_rn(-x, y, 1.0);
-  y = __fma_rn(y, e, y);
-  e = __fma_rn(-x, y, 1.0);
-  return __fma_rn(y, e, y);
+  const double e = __fma_rn(-x, y, 1.0);
+  const double t = __fma_rn(e, e, e);
+  return __fma_rn(y, t, y);
+}
+// reciprocals that only scale the step size (eq. 2): one Newton iteration, relative error ~ 2^-40 - the step size is a
+// free parameter of the scheme, and 1e-12 of it is far below the 1e-9 the results are compared at
+GRAY_DEV float vrcp_step(float x) { return srcp(x); }
+GRAY_DEV double vrcp_step(double x) {
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  return __fma_rn(y, __fma_rn(-x, y, 1.0), y);
 }
 GRAY_DEV f2 vrcp(f2 v) { float lo, hi; f2_unpack(v, lo, hi); return f2_pack(srcp(lo), srcp(hi)); }
+GRAY_DEV f2 vrcp_step(f2 v) { return vrcp(v); }
 
 // exact (IEEE) reciprocal for the scalar once-per-photon work of the reduced system
 GRAY_DEV float vrcp_exact(float x) { return __frcp_rn(x); }
