@@ -117,6 +117,9 @@ typedef struct {
  *   random  (alpha, beta) from the stateless generator of DESIGN.md keyed by (seed, p)
  *   position  r_obs o + alpha yhat + beta bhat,  o = (sin i, 0, cos i), bhat = (-cos i, 0, sin i)
  *   momentum  along +o, k^t from the null condition g_mu_nu k^mu k^nu = 0, normalised to E = -k_t = 1
+ * A pixel exactly on the spin axis (inc_deg = 0 or 180 and alpha = beta = 0) gets theta = 0 or pi and
+ * k^theta = k^phi = 0 (the limit); Boyer-Lindquist coordinates cannot carry such a ray and gray_integrate
+ * ends it GRAY_BAD on its first step.
  * Writes x, k, status = GRAY_LIVE, steps = 0 and the image-plane fields of *state.  Asynchronous.
  * Errors: GRAY_ERR_ARG, GRAY_ERR_DOMAIN (also when half_width is so large that a pixel starts
  * outside 1.01 r_obs), GRAY_ERR_CUDA.                                                               */
@@ -239,9 +242,15 @@ GRAY_API int gray_shadow_edge(const gray_state* state, int32_t n_angles, double*
  * rule on the n_theta spokes.  bridge_axis != 0 (n_theta odd): the middle spoke vartheta = pi/2 has alpha = 0, its rays
  * run through the spin axis, the degenerate case of Boyer-Lindquist coordinates in which the second-order equations
  * lose rays even with the xi monitor (R20); its radius is then replaced by the mean of its two neighbours
- * before the statistics are formed.  Requires a full polar batch.  radius_dev (n_theta doubles) may be NULL.
- * Synchronises the stream.                                                                             */
-typedef struct { double alpha_min, alpha_max, D, R_mean, A; } gray_ring_stats;
+ * before the statistics are formed; what the spoke's own rays gave is reported next to it (axis_radius_traced,
+ * axis_rays_lost), so a caller sees an interpolated value for what it is.  Requires a full polar batch.  radius_dev
+ * (n_theta doubles) may be NULL.  Synchronises the stream.                                                                             */
+typedef struct {
+  double alpha_min, alpha_max, D, R_mean, A;
+  double axis_radius_traced;   /* n_theta odd: ring radius on the axis spoke vartheta = pi/2 as the rays gave it ...        */
+  double axis_radius_used;     /* ... and the one the statistics used (the neighbours' mean if bridge_axis, else the same)  */
+  uint64_t axis_rays_lost;     /* rays of that spoke that ended neither CAPTURED nor ESCAPED (BAD, or LIVE at the cap)     */
+} gray_ring_stats;
 GRAY_API int gray_ring_polar(const gray_state* state, int32_t bridge_axis, double* radius_dev, gray_ring_stats* stats_host,
                     void* workspace_dev, size_t workspace_bytes, void* cuda_stream);
 

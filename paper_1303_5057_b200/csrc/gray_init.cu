@@ -66,13 +66,17 @@ __global__ void __launch_bounds__(256) init_kernel(const __grid_constant__ InitA
   const double q = sqrt(q2);
   const double r = sqrt(q2 + Z * Z);
   const double ct = Z / r, st = q / r;
-  const double th = acos(ct);
+  const double th = atan2(q, Z);              // well conditioned for observers near the spin axis, where acos(Z / r) is not
   const double ph = atan2(Y, X);
   // velocity o = (sin i, 0, cos i) in spherical components: o.rhat = r_obs / r,
   // o.thhat / r, o.phhat / (r sin th)
   double kr = A.r_obs / r;
   double kh = (A.sin_i * ct * (X / q) - A.cos_i * st) / r;
   double kp = -A.sin_i * Y / q2;
+  // A pixel exactly on the spin axis (q = 0: a face-on observer's central pixel) has no azimuth; o is then parallel to
+  // the axis and its theta and phi components vanish in the limit.  The state is finite; the ray itself cannot be
+  // followed in Boyer-Lindquist coordinates (1 / sin(theta) in the first right-hand side) and ends GRAY_BAD (gray.h).
+  if (q == 0.0) { kh = 0.0; kp = 0.0; }
   // null condition for k^t (future-directed root), then normalise to E = -k_t = 1
   const double a = A.a, a2 = a * a, r2 = r * r, s2 = st * st;
   const double Sg = r2 + a2 * ct * ct;

@@ -197,12 +197,26 @@ __global__ void __launch_bounds__(1024) ring_polar_kernel(const __grid_constant_
     var += ((k == 0 || k == A.n_theta - 1) ? 0.5 : 1.0) * d * d;
   }
   var = block_sum(var, sh) / (double)(A.n_theta - 1);
+  // the axis spoke (vartheta = pi/2, n_theta odd), reported whether or not it is bridged: its radius as traced, the
+  // radius used, and how many of its rays did not end CAPTURED or ESCAPED (gray.h)
+  const long long mid = (A.n_theta - 1) / 2;
+  const bool has_axis = A.n_theta >= 3 && (A.n_theta % 2) == 1;
+  double lost = 0.0;
+  if (has_axis)
+    for (long long j = threadIdx.x; j < A.n_R; j += blockDim.x) {
+      const uint8_t st = A.status[mid * A.n_R + j];
+      lost += (st != GRAY_CAPTURED && st != GRAY_ESCAPED) ? 1.0 : 0.0;
+    }
+  lost = block_sum(lost, sh);
   if (threadIdx.x == 0) {
     A.ws->stats[0] = amin;
     A.ws->stats[1] = amax;
     A.ws->stats[2] = fabs(amin + amax) / 2.0;
     A.ws->stats[3] = mean;
     A.ws->stats[4] = 2.0 * sqrt(var);
+    A.ws->stats[5] = has_axis ? ring_radius_raw(A, mid) : 0.0;
+    A.ws->stats[6] = has_axis ? ring_radius(A, mid) : 0.0;
+    A.ws->stats[7] = lost;
   }
 }
 
@@ -297,11 +311,12 @@ int gray_ring_polar(const gray_state* state, int32_t bridge_axis, double* radius
   A.R_lo = state->r_lo; A.R_hi = state->half_width; A.bridge_axis = bridge_axis; A.radius = radius_dev; A.ws = ws;
   ring_polar_kernel<<<1, 1024, 0, stream>>>(A);
   GRAY_CUDA(cudaGetLastError());
-  double s[5];
+  double s[8];
   GRAY_CUDA(cudaMemcpyAsync(s, &ws->stats[0], sizeof s, cudaMemcpyDeviceToHost, stream));
   GRAY_CUDA(cudaStreamSynchronize(stream));
   stats_host->alpha_min = s[0]; stats_host->alpha_max = s[1]; stats_host->D = s[2];
   stats_host->R_mean = s[3]; stats_host->A = s[4];
+  stats_host->axis_radius_traced = s[5]; stats_host->axis_radius_used = s[6]; stats_host->axis_rays_lost = (uint64_t)s[7];
   return GRAY_OK;
 }
 

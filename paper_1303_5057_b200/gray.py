@@ -44,7 +44,8 @@ class _Counters(C.Structure):
 
 
 class _RingStats(C.Structure):
-    _fields_ = [(k, C.c_double) for k in ("alpha_min", "alpha_max", "D", "R_mean", "A")]
+    _fields_ = [(k, C.c_double) for k in ("alpha_min", "alpha_max", "D", "R_mean", "A", "axis_radius_traced", "axis_radius_used")] + \
+               [("axis_rays_lost", C.c_uint64)]
 
 
 class _ShadowStats(C.Structure):
