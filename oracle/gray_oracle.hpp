@@ -38,11 +38,11 @@
 //                           the paper's fits eqs. 11-14 (soft)
 //   shadow statistics     : Bardeen closed-form curve (area, alpha extent, D,
 //                           <R>, A), an exact synthetic disc, paper eqs. 11-14
-// Parity unpinned (GPU-vs-oracle only): the final state of CAPTURED rays at
-// 1.01 r_h off the equatorial plane for a != 0 (a = 0: phi by the orbit integral, k^r by
-// the null condition; Kerr equatorial rays: phi, k^r by the Bardeen 1972 quadrature),
-// the EQ2 step rule's min() selection on individual steps, and the
-// Kerr (a != 0) equatorial crossing radius beyond the invariants above.
+//   Kerr rays off the equator: final (r, theta, phi) of CAPTURED and ESCAPED rays, and the equatorial
+//                           crossing (r, phi) of stop_at_equator, against Carter's separated first-order
+//                           equations in Mino time integrated by DOP853 (error falls 16x per step halving)
+// Parity unpinned (GPU-vs-oracle only): which branch of the EQ2 step rule's min() individual steps of a
+// whole trajectory take (the two branch values themselves are pinned by hand).
 #pragma once
 #include <cmath>
 #include <cstdint>

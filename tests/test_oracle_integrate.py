@@ -496,3 +496,85 @@ def test_equatorial_kerr_rays_against_the_bardeen_1972_quadrature():
         assert abs(y[5] - rdot(y[1])) < 2e-2 * rdot(y[1])
         checked += 1
     assert checked >= 4
+
+
+# ---- whole Kerr trajectories off the equatorial plane, against Carter's separated first-order equations ----------
+def _carter_flow(a, y0, events):
+    """The same geodesic from a different formulation: Carter's (1968) separated equations in Mino time tau
+    (dlambda = Sigma dtau) for the covariant momenta, with the constants E = -p_t, L = p_phi of the initial state:
+        dr/dtau = Delta p_r,      dp_r/dtau  = -(r - 1) p_r^2 + 2 r E R0 / Delta - (r - 1) R0^2 / Delta^2,   R0 = (r^2 + a^2) E - a L,
+        dth/dtau = p_th,          dp_th/dtau = (L/s - a E s)(L c / s^2 + a E c),
+        dphi/dtau = a R0 / Delta - a E + L / s^2
+    (no Christoffel symbols, no second-order equations), integrated by scipy's DOP853 at 1e-13 towards negative tau
+    (the oracle steps dlambda < 0) until `events` (terminal) fires.  Returns the solve_ivp result."""
+    from scipy.integrate import solve_ivp
+    E, L, _, _ = o.invariants(a, y0)
+    r, th = y0[1], y0[2]
+    Sg, Dl = r * r + (a * np.cos(th)) ** 2, r * r - 2 * r + a * a
+    z0 = np.array([r, th, y0[3], Sg / Dl * y0[5], Sg * y0[6]])
+
+    def f(tau, z):
+        r, th, ph, pr, pt = z
+        s, c = np.sin(th), np.cos(th)
+        Dl = r * r - 2 * r + a * a
+        R0 = (r * r + a * a) * E - a * L
+        return [Dl * pr, pt, a * R0 / Dl - a * E + L / (s * s),
+                -(r - 1) * pr * pr + 2 * r * E * R0 / Dl - (r - 1) * R0 * R0 / (Dl * Dl),
+                (L / s - a * E * s) * (L * c / (s * s) + a * E * c)]
+
+    guard = lambda tau, z: z[0] - 1.003 * o.horizon(a)      # the equations are singular on the horizon: stop short of it
+    guard.terminal = True
+    return solve_ivp(f, (0.0, -1e3), z0, method="DOP853", rtol=1e-13, atol=1e-14, events=[events, guard])
+
+
+def test_kerr_rays_off_the_equator_against_carters_separated_equations():
+    # The final state of whole Kerr (a != 0) trajectories away from the equatorial plane, CAPTURED ones (stopped at the
+    # first step below 1.01 r_h) and ESCAPED ones: the oracle's final (r, theta, phi) must lie on the geodesic that
+    # Carter's first-order equations give for the same initial state - theta and phi compared where that solution
+    # reaches the oracle's final radius - to the RK4 scheme's truncation error, which falls ~16x when h is halved.
+    a = 0.9
+    rh = o.horizon(a)
+    seen = {o.CAPTURED: 0, o.ESCAPED: 0}
+    for inc, al, be in [(60.0, 1.0, 2.0), (60.0, -1.5, -3.0), (30.0, 2.0, 1.0), (75.0, 0.5, -2.5), (60.0, 6.0, 5.0), (45.0, -7.0, 3.0),
+                        (60.0, 3.5, 6.5)]:
+        y0 = o.init_ray(a, 1000.0, inc, al, be)
+        errs = []
+        for h in (1 / 32, 1 / 64):
+            y, st, n = o.integrate(a, y0, h, 1.01 * rh, 1010.0, o.STEP_EQ2, 40000)
+            assert st in seen
+            if st == o.CAPTURED:
+                ev = lambda tau, z, rf=y[1]: z[0] - rf            # inward all the way: the first crossing of r_f
+                ev.direction = 0
+            else:
+                ev = lambda tau, z, rf=y[1]: z[0] - rf if tau < -1e-6 else -1.0      # outbound crossing, after the periapsis
+                ev.direction = 0
+            ev.terminal = True
+            sol = _carter_flow(a, y0, ev)
+            assert sol.status == 1 and len(sol.y_events[0]) == 1, (inc, al, be, st)
+            rE, thE, phE = sol.y_events[0][0][:3]
+            assert abs(rE - y[1]) < 1e-9 * y[1]
+            errs.append(max(abs(y[2] - thE), abs(y[3] - phE)))
+        seen[st] += 1
+        assert errs[0] < 1e-5, (inc, al, be, st, errs)                       # h = 1/32: the scheme's truncation error
+        assert errs[1] < errs[0] / 10, (inc, al, be, st, errs)      # and it falls at ~4th order
+    assert seen[o.CAPTURED] >= 3 and seen[o.ESCAPED] >= 3, seen
+
+
+def test_equatorial_projection_kerr_crossing_against_carters_separated_equations():
+    # The Kerr equatorial-plane crossing of stop_at_equator (R19): (r, phi) of the landed state against the point where
+    # the solution of Carter's first-order equations first reaches theta = pi/2.
+    a = 0.95
+    for inc, al, be in [(60.0, 5.0, 8.0), (60.0, -7.0, 6.0), (60.0, 9.0, -9.0), (30.0, 2.0, 9.0), (80.0, -3.0, 4.0)]:
+        y0 = o.init_ray(a, 1000.0, inc, al, be)
+        ev = lambda tau, z: z[1] - np.pi / 2
+        ev.terminal, ev.direction = True, 0
+        sol = _carter_flow(a, y0, ev)
+        assert sol.status == 1 and len(sol.y_events[0]) == 1
+        rE, _, phE = sol.y_events[0][0][:3]
+        errs = []
+        for h in (1 / 32, 1 / 64):
+            y, st, n = o.integrate(a, y0, h, 1.01 * o.horizon(a), 1010.0, o.STEP_EQ2, 40000, stop_at_equator=True)
+            assert st == o.EQUATOR and abs(y[2] - np.pi / 2) < 1e-8
+            errs.append(max(abs(y[1] - rE) / rE, abs(y[3] - phE)))
+        assert errs[0] < 1e-5, (inc, al, be, errs)
+        assert errs[1] < errs[0] / 6 or errs[1] < 2e-8, (inc, al, be, errs)
