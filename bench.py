@@ -191,13 +191,14 @@ def ncu_dram_bytes_per_photon():
     return None, None
 
 
-def executed_flops_per_photon_step(variant):
-    """FP operations the kernel variant EXECUTES per photon-step (FMA = 2), from the per-opcode executed-instruction
-    counts of the committed ncu captures (profiles/r02_executed_ops.csv); None if the variant was not captured."""
+def executed_flops_per_lane_step(variant):
+    """FP operations the kernel variant EXECUTES per issued lane-step (one RK4 step of one photon slot, whether or not
+    the slot holds a live photon; FMA = 2), from the per-opcode executed thread-instruction counts of the committed ncu
+    captures (profiles/r02_executed_ops.csv); None if the variant was not captured."""
     rows = read_profile_csv("r02_executed_ops.csv")
     for r in rows or []:
         if r["variant"] == variant:
-            return float(r["flops_per_photon_step"])
+            return float(r["flops_per_issued_lane_step"])
     return None
 
 
@@ -331,10 +332,11 @@ class Runner:
         flops = FLOPS_PER_PHOTON_STEP[m["rule"]]
         reduced = m["system"] == "reduced"
         achieved = None if reduced else flops * rate / 1e12
-        exe = executed_flops_per_photon_step(variant_name(m["prec"], m["rule"], m["case"], m["xi_eps"], m["system"], m["ppt"]))
+        exe = executed_flops_per_lane_step(variant_name(m["prec"], m["rule"], m["case"], m["xi_eps"], m["system"], m["ppt"]))
+        issued_rate = m["issued"] / self.world / m["steps"] / (m["kernel_ms"] * 1e-3)       # lane-steps per second inside the kernel
         return dict(achieved=achieved, peak=peak, frac=None if reduced else achieved / peak,
-                    executed_flops_per_photon_step=exe, achieved_executed=exe * rate / 1e12 if exe else None,
-                    frac_executed=exe * rate / 1e12 / peak if exe else None,
+                    executed_flops_per_lane_step=exe, achieved_executed=exe * issued_rate / 1e12 if exe else None,
+                    frac_executed=exe * issued_rate / 1e12 / peak if exe else None,
                     frac_survey_hand_tally=None if (reduced or m["prec"] != "f32") else FLOPS_SURVEY_HAND_TALLY * rate / 1e12 / peak,
                     kernel_ms=m["kernel_ms"], kernel_share_of_step=m["kernel_ms"] * m["steps"] / m["ms"],
                     lane_efficiency=m["photon_steps"] / m["issued"] if m["issued"] else None)
@@ -471,8 +473,9 @@ def run_gray(args):
                                    "x photons of this launch") if dram_b else None,
                 "kernel": "gray::integrate_kernel", "kernel_ms": rf["kernel_ms"], "kernel_share_of_step": rf["kernel_share_of_step"],
                 "flops_per_photon_step": flops, "flops_source": "oracle operation tally (add=sub=mul=div=sqrt=sin=cos=1): BASELINE's definition",
-                "executed_flops_per_photon_step": rf["executed_flops_per_photon_step"],
-                "executed_source": "ncu per-opcode executed instruction counts (profiles/r02_executed_ops.csv), FMA = 2",
+                "executed_flops_per_lane_step": rf["executed_flops_per_lane_step"],
+                "executed_source": "ncu per-opcode executed thread-instruction counts per issued lane-step (profiles/r02_executed_ops.csv), "
+                                   "FMA = 2, x issued lane-steps of this run",
                 "achieved_executed": rf["achieved_executed"], "frac_executed": rf["frac_executed"],
                 "flops_survey_hand_tally": FLOPS_SURVEY_HAND_TALLY, "frac_survey_hand_tally": rf["frac_survey_hand_tally"],
                 "peak_source": "148 SMs x %d lanes x 2 x 1.965 GHz (DESIGN.md)" % (128 if args.prec == "f32" else 64),

@@ -56,3 +56,9 @@ def test_profile_csv_readers():
     assert bench.variant_name("f32", "eq2", "realistic", 0.0, "full", 0) == "f32_eq2"
     assert bench.variant_name("f64", "eq2", "realistic", 1e-3, "full", 0) == "f64_eq2_xi"
     assert bench.variant_name("f32", "rel", "peak", 0.0, "full", 0) == "f32_rel_frozen"
+    # executed FP operations per issued lane-step (ncu): below the oracle's nominal tally, above the FMA-only floor
+    for variant, lo, hi in (("f32_eq2", 400, 787), ("f64_eq2", 500, 787), ("f32_eq2_xi", 450, 900), ("f32_rel_frozen", 400, 777),
+                            ("f32x1_eq2", 400, 787)):
+        e = bench.executed_flops_per_lane_step(variant)
+        assert e is not None and lo < e < hi, (variant, e)
+    assert bench.executed_flops_per_lane_step("no_such_variant") is None
