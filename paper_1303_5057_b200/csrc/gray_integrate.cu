@@ -44,6 +44,10 @@ struct IntegrateArgs {
 #ifndef GRAY_BLOCK
 #define GRAY_BLOCK 128
 #endif
+#ifndef GRAY_STEP_UNROLL
+#define GRAY_STEP_UNROLL 2     // RK4 steps per trip of the inner loop (refill_interval is rounded up to a multiple): two copies of the
+                               // step let the new state of one be the old state of the other without register moves
+#endif
 #ifndef GRAY_F2_MIN_BLOCKS
 #define GRAY_F2_MIN_BLOCKS 4
 #endif
@@ -211,7 +215,9 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
       if (exhausted) break;
       continue;
     }
-    for (int it = 0; it < A.refill_interval; ++it) {
+    for (int it2 = 0; it2 < A.refill_interval; it2 += GRAY_STEP_UNROLL)
+#pragma unroll
+    for (int un = 0; un < GRAY_STEP_UNROLL; ++un) {
       any = false;
 #pragma unroll
       for (int l = 0; l < N; ++l) any |= have[l];
@@ -333,7 +339,7 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
         }
       }
     }
-    c_iter += A.refill_interval;
+    c_iter += (A.refill_interval + GRAY_STEP_UNROLL - 1) / GRAY_STEP_UNROLL * GRAY_STEP_UNROLL;
   }
 
   c_steps = warp_sum(c_steps);

@@ -7,17 +7,15 @@
 // App. A.3).  They are not evaluated symbol by symbol.  With
 //     Sigma = r^2 + a^2 cos^2(th),  Delta = (r - r_+)(r - r_-),  P = r^2 - a^2 cos^2(th),
 //     rho = r^2 + a^2,  s = sin(th),  c = cos(th),
-//     u = k^t - a s^2 k^phi,        w = a k^t - rho k^phi
+//     q = (k^t - a s^2 k^phi) / Sigma,        v = k^phi - a q   (= (rho k^phi - a k^t) / Sigma)
 // the contractions -Gamma^mu_ab k^a k^b collapse to:
-//   dk^t  /dl = -2/Sigma^2 [ (k^r/Delta) (rho P u - 2 a s^2 r^2 Sigma k^phi) - 2 a^2 r s c k^th u ]
-//   dk^phi/dl = -2/Sigma^2 [ (k^r/Delta) (a P u + r Sigma (Sigma - 2r) k^phi)
-//                            + (c/s) k^th (Sigma^2 k^phi - 2 a r u) ]
+//   dk^t  /dl = -2/Sigma [ (k^r/Delta) (rho P q - 2 a s^2 r^2 k^phi) - 2 a^2 r s c k^th q ]
+//   dk^phi/dl = -2/Sigma [ (k^r/Delta) (a P q + r (Sigma - 2r) k^phi) + (c/s) k^th (Sigma k^phi - 2 a r q) ]
 //   dk^r  /dl = (k^r)^2 [ (r - 1)/Delta - r/Sigma ]
-//               + 1/Sigma [ Delta (r (s^2 (k^phi)^2 + (k^th)^2) - P u^2/Sigma^2) + 2 a^2 s c k^r k^th ]
-//   dk^th /dl = 1/Sigma [ s c (2 r w^2/Sigma^2 + Delta (k^phi)^2 + a^2 ((k^th)^2 - (k^r)^2/Delta))
-//                         - 2 r k^r k^th ]
-// One sincos and three reciprocals (1/Sigma, 1/Delta, 1/s) per evaluation; 66 FP-pipe operations
-// (27 of them fused multiply-adds) besides the 13 of the sincos.
+//               + 1/Sigma [ Delta (r (s^2 (k^phi)^2 + (k^th)^2) - P q^2) + 2 a^2 s c k^r k^th ]
+//   dk^th /dl = 1/Sigma [ s c (2 r v^2 + Delta (k^phi)^2 + a^2 ((k^th)^2 - (k^r)^2/Delta)) - 2 r k^r k^th ]
+// Three reciprocals (1/Sigma, 1/Delta, 1/s) and 63 FP-pipe operations (26 of them fused multiply-adds) per
+// evaluation, besides the sine and cosine.
 //
 // Conditioning: inside the kernel the radial variable is the height above
 // the horizon  d = r - r_+  (so Delta = d (d + r_+ - r_-) keeps full relative precision where the
@@ -52,6 +50,8 @@ struct Consts {
   V nsixth, r24;                                   // sincos_rotate (float builds): -1/6, 1/24
   S r_cap, r_esc;                         // termination radii, as heights above the horizon (r - r_+): the kernel's radial variable
   S xi_eps;                               // epsilon of the xi monitor (paper eq. 4); 0 = off
+  int stage2_in_range;                    // h / 2 <= RotateMax: under the eq. (2) rule the theta offset of stage 2, dl/2 k^th with
+                                          // |dl k^th| <= h, needs no range test before the angle-addition formulas (sincos_stage)
 };
 
 template <typename V>
@@ -75,6 +75,7 @@ __host__ inline Consts<V> make_consts(double a, double h, double r_cap, double r
   K.fc5 = B(-2.5585777763e-07);
   K.nsixth = B(-1.0 / 6.0); K.r24 = B(1.0 / 24.0);
   K.r_cap = (S)(r_cap - (1.0 + root)); K.r_esc = (S)(r_esc - (1.0 + root));   // differences formed in double
+  K.stage2_in_range = 0.5 * h * 1.001 <= (sizeof(S) == 4 ? 0.045 : 0.125);
   return K;
 }
 
@@ -205,16 +206,18 @@ __device__ __noinline__ double2 sincos_wide(double th0, double dlt) { double2 r;
 // sine and cosine of th0 + dlt for a stage, from (s0, c0) = (sin, cos)(th0).  Each photon by its own |dlt| (its
 // result must not depend on the photon it shares a thread with): the rotation within the series' range, else
 // sincos_wide.  A NaN dlt goes through the rotation and comes out NaN.
+// check = false (uniform over the launch): the caller knows that |dlt| is within the range (no test, rotation only).
 template <typename V>
-GRAY_DEV void sincos_stage(const Consts<V>& K, V th0, V s0, V c0, V dlt, V& s, V& c) {
+GRAY_DEV void sincos_stage(const Consts<V>& K, V th0, V s0, V c0, V dlt, V& s, V& c, bool check = true) {
   using S = typename VT<V>::S;
   constexpr int N = VT<V>::N;
+  sincos_rotate(K, s0, c0, dlt, s, c);
+  if (!check) return;
   S a[N];
   vunpack(dlt, a);
   bool wide = false;
 #pragma unroll
   for (int l = 0; l < N; ++l) wide |= sabs(a[l]) > RotateMax<S>::value;
-  sincos_rotate(K, s0, c0, dlt, s, c);
   if (wide) {
     S sr[N], cr[N], tb[N];
     vunpack(s, sr); vunpack(c, cr); vunpack(th0, tb);
@@ -241,40 +244,40 @@ GRAY_DEV void geodesic_accel(const Consts<V>& K, V d, V s, V c, V kt, V kr, V kh
   const V Dl = vmul(d, vadd(d, K.rpm));         // Delta = (r - r_+)(r - r_-): no cancellation at the horizon
   const V iS = vrcp(Sg), iD = vrcp(Dl), is = vrcp(s);
   const V niS = vneg(iS);
+  const V tniS = vadd(niS, niS);                // -2/Sigma
   const V s2 = vmul(s, s);
   const V sc = vmul(s, c);
   const V as2n = vmul(K.na, s2);                // -a s^2
   const V u = vfma(as2n, kp, kt);
+  const V q = vmul(u, iS);                      // u / Sigma
   const V krD = vmul(kr, iD);                   // k^r / Delta
-  const V niS2 = vmul(iS, niS);                 // -1/Sigma^2
-  const V tiS2 = vadd(niS2, niS2);              // -2/Sigma^2
-  const V Pu = vmul(P, u);
+  const V Pq = vmul(P, q);
+  const V rk = vmul(r, kp);
+  const V rq = vmul(r, q);
   const V Sgk = vmul(Sg, kp);
-  const V rSgk = vmul(r, Sgk);
-  const V ru = vmul(r, u);
-  // dk^t
-  const V e1 = vfma(K.two, vmul(vmul(as2n, r), rSgk), vmul(rho, Pu));
+  // dk^t = -2/Sigma [ (k^r/Delta) (rho P q - 2 a s^2 r^2 k^phi) - 2 a^2 r s c k^th q ]
+  const V e1 = vfma(K.two, vmul(vmul(as2n, r), rk), vmul(rho, Pq));
   const V tk = vmul(sc, kh);
-  const V Xt = vfma(K.n2a2, vmul(ru, tk), vmul(krD, e1));
-  out[0] = ACC ? vfma(tiS2, Xt, add[0]) : vmul(tiS2, Xt);
-  // dk^phi
-  const V e2 = vfma(K.a, Pu, vmul(vfma(K.m2, r, Sg), rSgk));
-  const V e3 = vfma(K.n2a, ru, vmul(Sg, Sgk));
+  const V Xt = vfma(K.n2a2, vmul(rq, tk), vmul(krD, e1));
+  out[0] = ACC ? vfma(tniS, Xt, add[0]) : vmul(tniS, Xt);
+  // dk^phi = -2/Sigma [ (k^r/Delta) (a P q + r (Sigma - 2r) k^phi) + (c/s) k^th (Sigma k^phi - 2 a r q) ]
+  const V e2 = vfma(K.a, Pq, vmul(vfma(K.m2, r, Sg), rk));
+  const V e3 = vfma(K.n2a, rq, Sgk);
   const V ck = vmul(vmul(c, is), kh);
   const V Xp = vfma(ck, e3, vmul(krD, e2));
-  out[3] = ACC ? vfma(tiS2, Xp, add[3]) : vmul(tiS2, Xp);
-  // dk^r
+  out[3] = ACC ? vfma(tniS, Xp, add[3]) : vmul(tniS, Xp);
+  // dk^r = (k^r)^2 [(r - 1)/Delta - r/Sigma] + 1/Sigma [ Delta (r (s^2 (k^phi)^2 + (k^th)^2) - P q^2) + 2 a^2 s c k^r k^th ]
   const V krkr = vmul(kr, kr);
   const V G = vfma(vadd(d, K.rpm1), iD, vmul(r, niS));      // (r - 1)/Delta - r/Sigma
   const V kp2 = vmul(kp, kp), kh2 = vmul(kh, kh);
   const V rA1 = vmul(r, vfma(s2, kp2, kh2));
-  const V Bp = vfma(vmul(Pu, u), niS2, rA1);
+  const V Bp = vfma(vneg(Pq), q, rA1);
   const V J2 = vfma(K.twoa2, vmul(tk, kr), vmul(Dl, Bp));
   out[1] = vfma(krkr, G, ACC ? vfma(iS, J2, add[1]) : vmul(iS, J2));
-  // dk^theta
-  const V w = vfma(K.na, u, Sgk);                           // rho k^phi - a k^t  (= Sigma k^phi - a u)
-  const V z2 = vfma(K.a2, vfma(vneg(krD), kr, kh2), vmul(Dl, kp2));     // Delta (k^phi)^2 + a^2 ((k^th)^2 - (k^r)^2 / Delta)
-  const V z3 = vfma(vmul(r, vmul(w, w)), vneg(tiS2), z2);
+  // dk^theta = 1/Sigma [ s c (2 r v^2 + Delta (k^phi)^2 + a^2 ((k^th)^2 - (k^r)^2 / Delta)) - 2 r k^r k^th ],  v = w/Sigma = k^phi - a q
+  const V v = vfma(K.na, q, kp);
+  const V z2 = vfma(K.a2, vfma(vneg(krD), kr, kh2), vmul(Dl, kp2));
+  const V z3 = vfma(K.two, vmul(r, vmul(v, v)), z2);
   const V z5 = vfma(K.m2, vmul(vmul(r, kr), kh), vmul(sc, z3));
   out[2] = ACC ? vfma(iS, z5, add[2]) : vmul(iS, z5);
 }
@@ -294,16 +297,17 @@ GRAY_DEV V step_size(const Consts<V>& K, V d, V kr, V kh, V kp) {
   return vmax(d1, d2);
 }
 
-// ---- state update y <- y + scale * rate --------------------------------------------------------------
+// ---- state update y <- y + scale * rate (scale_x for the four positions, scale_k for the four momenta) ----
 // `comp` carries, for the float builds, the rounding error of each update into the next one (compensated
 // summation): y + comp is the state to roughly twice the working precision.
 template <bool MASKED = false, typename V>
-GRAY_DEV void advance_state(const V y[8], const V comp[8], V scale, const V rate[8], V yn[8], V cn[8],
+GRAY_DEV void advance_state(const V y[8], const V comp[8], V scale_x, V scale_k, const V rate[8], V yn[8], V cn[8],
                             const bool* adv = nullptr) {
   using S = typename VT<V>::S;
   constexpr int N = VT<V>::N;
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
+    const V scale = i < 4 ? scale_x : scale_k;
     if (sizeof(typename VT<V>::S) == 4 && ((GRAY_COMP_MASK >> i) & 1)) {
       const V inc = vfma(scale, rate[i], comp[i]);
       const V s = vadd(y[i], inc);
@@ -367,6 +371,7 @@ GRAY_DEV void rk4_step(const Consts<V>& K, V y[8], V comp[8], V dl, bool rejecte
   constexpr int N = VT<V>::N;
   V acc[8], w[8], f[4], f1[4];
   const V hdl = vmul(K.half, dl);
+  const V dl6 = vmul(K.sixth, dl);
   // stage 1
   V s0, c0, ss, cc;
   if (FOLDED) sincos_folded(K, y[2], s0, c0);
@@ -380,11 +385,12 @@ GRAY_DEV void rk4_step(const Consts<V>& K, V y[8], V comp[8], V dl, bool rejecte
     w[i] = i == 2 ? vmul(hdl, y[6]) : vfma(hdl, y[4 + i], y[i]);      // w[2]: the stage's offset in theta, not theta
     w[4 + i] = vfma(hdl, f[i], y[4 + i]);
   }
-  // stages 2 and 3
+  // stages 2 and 3.  Stage 2 under the eq. (2) rule (FOLDED): |dl k^th| <= h by the rule itself, so with h / 2 inside the
+  // rotation's range (Consts::stage2_in_range) its offset needs no range test
 #pragma unroll
   for (int stage = 2; stage <= 3; ++stage) {
     const V hs = stage == 2 ? hdl : dl;
-    sincos_stage(K, y[2], s0, c0, w[2], ss, cc);
+    sincos_stage(K, y[2], s0, c0, w[2], ss, cc, !(stage == 2 && FOLDED && K.stage2_in_range));
     geodesic_accel<false>(K, w[1], ss, cc, w[4], w[5], w[6], w[7], (const V*)nullptr, f);
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
@@ -401,7 +407,7 @@ GRAY_DEV void rk4_step(const Consts<V>& K, V y[8], V comp[8], V dl, bool rejecte
   sincos_stage(K, y[2], s0, c0, w[2], ss, cc);
   geodesic_accel<true>(K, w[1], ss, cc, w[4], w[5], w[6], w[7], acc + 4, acc + 4);
   V yn[8], cn[8];
-  advance_state<MASKED>(y, comp, vmul(K.sixth, dl), acc, yn, cn, adv);
+  advance_state<MASKED>(y, comp, dl6, dl6, acc, yn, cn, adv);
 #pragma unroll
   for (int l = 0; l < N; ++l) rejected[l] = false;
   if (XI) {
@@ -419,10 +425,11 @@ GRAY_DEV void rk4_step(const Consts<V>& K, V y[8], V comp[8], V dl, bool rejecte
       any |= rejected[l];
     }
     if (any) {
-      V rate[8], ye[8], ce[8];
+      V re[8], ye[8], ce[8];
 #pragma unroll
-      for (int i = 0; i < 4; ++i) { rate[i] = y[4 + i]; rate[4 + i] = f1[i]; }
-      advance_state(y, comp, vmul(K.ninth, dl), rate, ye, ce);
+      for (int i = 0; i < 4; ++i) { re[i] = y[4 + i]; re[4 + i] = f1[i]; }
+      const V dl9 = vmul(K.ninth, dl);
+      advance_state(y, comp, dl9, dl9, re, ye, ce);
 #pragma unroll
       for (int i = 0; i < 8; ++i) {
         S a[N], b[N], ca[N], cb[N];
@@ -442,7 +449,7 @@ GRAY_DEV void rk4_step(const Consts<V>& K, V y[8], V comp[8], V dl, bool rejecte
 //   u = k^t - a s^2 k^phi = (rho E - a L)/Delta,    w = Sigma k^phi - a u = L/s^2 - a E,
 //   k^phi = (w + a u)/Sigma,                        k^t = u + a s^2 k^phi
 // (the inverse Kerr metric applied to (-E, L), regrouped), and dk^r/dl, dk^theta/dl are the same expressions as
-// in geodesic_accel.  51 FP-pipe operations besides the sincos, against 66.
+// in geodesic_accel.  49 FP-pipe operations besides the sincos, against 63.
 // ======================================================================================================
 GRAY_DEV void sincos_s(float x, float& s, float& c) { sincosf(x, &s, &c); }
 GRAY_DEV void sincos_s(double x, double& s, double& c) { sincos(x, &s, &c); }
@@ -495,24 +502,24 @@ GRAY_DEV void geodesic_accel_reduced(const Consts<V>& K, V d, V s, V c, V kr, V 
   const V sc = vmul(s, c);
   const V u = vmul(vfma(rho, E, naL), iD);
   const V w = vfma(L, vmul(is, is), naE);
-  kp = vmul(vfma(K.a, u, w), iS);
+  const V q = vmul(u, iS);                      // u / Sigma
+  const V v = vmul(w, iS);                      // w / Sigma
+  kp = vfma(K.a, q, v);
   kt = vfma(vmul(K.a, s2), kp, u);
   const V krD = vmul(kr, iD);
-  const V niS2 = vmul(iS, niS);
-  const V tiS2 = vadd(niS2, niS2);
-  const V Pu = vmul(P, u);
+  const V Pq = vmul(P, q);
   const V tk = vmul(sc, kh);
   // dk^r
   const V krkr = vmul(kr, kr);
   const V G = vfma(vadd(d, K.rpm1), iD, vmul(r, niS));
   const V kp2 = vmul(kp, kp), kh2 = vmul(kh, kh);
   const V rA1 = vmul(r, vfma(s2, kp2, kh2));
-  const V Bp = vfma(vmul(Pu, u), niS2, rA1);
+  const V Bp = vfma(vneg(Pq), q, rA1);
   const V J2 = vfma(K.twoa2, vmul(tk, kr), vmul(Dl, Bp));
   out[0] = vfma(krkr, G, ACC ? vfma(iS, J2, add[0]) : vmul(iS, J2));
   // dk^theta
   const V z2 = vfma(K.a2, vfma(vneg(krD), kr, kh2), vmul(Dl, kp2));     // Delta (k^phi)^2 + a^2 ((k^th)^2 - (k^r)^2 / Delta)
-  const V z3 = vfma(vmul(r, vmul(w, w)), vneg(tiS2), z2);
+  const V z3 = vfma(K.two, vmul(r, vmul(v, v)), z2);
   const V z5 = vfma(K.m2, vmul(vmul(r, kr), kh), vmul(sc, z3));
   out[1] = ACC ? vfma(iS, z5, add[1]) : vmul(iS, z5);
 }
