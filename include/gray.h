@@ -144,8 +144,8 @@ typedef struct {
   double r_escape_factor;    /* escaped when r > factor * r_obs (configs: 1.01)                       */
   int32_t rule;              /* gray_step_rule                                                        */
   int32_t schedule;          /* gray_schedule                                                         */
-  int32_t refill_interval;   /* REFILL: RK4 steps between looks at the termination mask (>= 1; 0 = default 8; odd values are
-                                rounded up to the next even number: the kernel takes its steps in pairs) */
+  int32_t refill_interval;   /* REFILL: RK4 steps between looks at the termination mask (>= 1; 0 = default 8; the full-system
+                                kernels take their steps in pairs and round odd values up) */
   int32_t frozen;            /* peak-rate case of BASELINE config 4 (reading R17): every
                                 live photon is stepped until its counter reaches max_steps with no
                                 early exit; once a test fires its state, status and step count are

@@ -35,6 +35,11 @@
 
 namespace gray {
 
+// Largest |dlt| for which sincos_rotate's series are used (beyond it: sincos_wide)
+template <typename S> struct RotateMax;
+template <> struct RotateMax<float> { static constexpr float value = 0.045f; };
+template <> struct RotateMax<double> { static constexpr double value = 0.04; };
+
 // Constants of a launch, already broadcast to V (for f2 both halves hold the same number, so the packed
 // instructions can take them straight from the constant bank / uniform registers).
 template <typename V>
@@ -75,7 +80,7 @@ __host__ inline Consts<V> make_consts(double a, double h, double r_cap, double r
   K.fc5 = B(-2.5585777763e-07);
   K.nsixth = B(-1.0 / 6.0); K.r24 = B(1.0 / 24.0);
   K.r_cap = (S)(r_cap - (1.0 + root)); K.r_esc = (S)(r_esc - (1.0 + root));   // differences formed in double
-  K.stage2_in_range = 0.5 * h * 1.001 <= (sizeof(S) == 4 ? 0.045 : 0.125);
+  K.stage2_in_range = 0.5 * h * 1.001 <= (double)RotateMax<S>::value;
   return K;
 }
 
@@ -168,11 +173,9 @@ GRAY_DEV void sincos_folded<double>(const Consts<double>& K, double x, double& s
 
 // (s, c) = (sin, cos)(th0 + dlt) from (s0, c0) = (sin, cos)(th0):  s = s0 + c0 sd + s0 cm,  c = c0 - s0 sd + c0 cm
 // with sd = sin(dlt), cm = cos(dlt) - 1 by their Taylor series.  float: sd = dlt - dlt^3/6, cm = -dlt^2/2 + dlt^4/24
-// (9 operations; truncation < 3.4e-8 relative for |dlt| <= kRotateMax).  double: through dlt^9 / dlt^10
-// (15 operations; < 3e-17 for |dlt| <= 1/8).
-template <typename S> struct RotateMax;
-template <> struct RotateMax<float> { static constexpr float value = 0.045f; };
-template <> struct RotateMax<double> { static constexpr double value = 0.125; };
+// (9 operations; truncation < 3.4e-8 relative for |dlt| <= RotateMax).  double: through dlt^7 / dlt^8
+// (13 operations; truncation dlt^8 / 9! < 2e-17 relative for |dlt| <= RotateMax = 0.04; under eq. (2) with h = 1/32 the
+// stage offsets stay below 1/32).
 template <typename V>
 GRAY_DEV void sincos_rotate(const Consts<V>& K, V s0, V c0, V dlt, V& s, V& c) {
   const V u = vmul(dlt, dlt);
@@ -184,13 +187,11 @@ GRAY_DEV void sincos_rotate(const Consts<V>& K, V s0, V c0, V dlt, V& s, V& c) {
 template <>
 GRAY_DEV void sincos_rotate<double>(const Consts<double>&, double s0, double c0, double dlt, double& s, double& c) {
   const double u = __dmul_rn(dlt, dlt);
-  double sp = 2.7557319223985890653e-06;                        //  1/9!
-  sp = __fma_rn(sp, u, -1.9841269841269841270e-04);             // -1/7!
+  double sp = -1.9841269841269841270e-04;                       // -1/7!
   sp = __fma_rn(sp, u, 8.3333333333333332177e-03);              //  1/5!
   sp = __fma_rn(sp, u, -1.6666666666666665741e-01);             // -1/3!
   const double sd = __fma_rn(__dmul_rn(dlt, u), sp, dlt);
-  double cp = -2.7557319223985888276e-07;                       // -1/10!
-  cp = __fma_rn(cp, u, 2.4801587301587301566e-05);              //  1/8!
+  double cp = 2.4801587301587301566e-05;                        //  1/8!
   cp = __fma_rn(cp, u, -1.3888888888888889419e-03);             // -1/6!
   cp = __fma_rn(cp, u, 4.1666666666666664354e-02);              //  1/4!
   cp = __fma_rn(cp, u, -0.5);
