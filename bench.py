@@ -464,7 +464,9 @@ def run_gray(args):
     if args.prec == "f32" and args.photons_per_thread != 1:
         lane_peak = 148 * 128 * 1.965e9
         mix = {"ffma2_invariant_operands": g.gray_packed_peak(0) / lane_peak, "ffma2_three_register_pairs": g.gray_packed_peak(1) / lane_peak,
-               "integrator_mix_r01": g.gray_packed_peak(2) / lane_peak}
+               "ffma2_two_register_pairs": g.gray_packed_peak(4) / lane_peak, "fmul2_two_register_pairs": g.gray_packed_peak(3) / lane_peak,
+               "integrator_mix_r01": g.gray_packed_peak(2) / lane_peak, "integrator_packed_mix": g.gray_packed_peak(5) / lane_peak,
+               "integrator_packed_mix_with_its_other_instructions": g.gray_packed_peak(6) / lane_peak}
     dram_b, dram_src = ncu_dram_bytes_per_photon()
     flops = FLOPS_PER_PHOTON_STEP[args.rule]
     roofline = {"bound": "alu", "achieved": rf["achieved"], "peak": rf["peak"], "unit": "TFLOP/s", "frac": rf["frac"],

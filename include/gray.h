@@ -287,8 +287,14 @@ GRAY_API int gray_fma_peak(int32_t prec, int32_t iters, double* flops_per_s_host
  * the FFMA peak.
  *   mix 0  FFMA2 x <- x * m + c with loop-invariant m, c
  *   mix 1  FFMA2 reading three different, changing register pairs
- *   mix 2  the integrator's instruction mix: 50 % FMUL2, 37.5 % FFMA2 (three pairs), 12.5 % FADD2
- * Returns fp32 lane-operations per second (one FFMA2 = 2 per thread; multiply by 2 for FMA flops of mix 0 / 1).
+ *   mix 2  round 1's instruction mix: 50 % FMUL2, 37.5 % FFMA2 (three pairs), 12.5 % FADD2
+ *   mix 3  FMUL2 reading two changing pairs            mix 4  FFMA2 x <- x * x' + x (two distinct pairs)
+ *   mix 5  the full-system integrator's packed instructions as they stand (per 16: 7 FMUL2, 3 FFMA2 with three pairs,
+ *          3 FFMA2 with two pairs and a launch constant, 2 FADD2, 1 FADD2 with a constant)
+ *   mix 6  mix 5 plus the other instructions the integrator issues beside them (per 16 packed: ~1.2 MUFU.RCP and
+ *          ~5 integer / select / move instructions): the rate the integrator's loop can reach at best
+ * Returns packed fp32 lane-operations per second (one packed instruction = 2 per thread; multiply by 2 for FMA flops of
+ * mix 0 / 1 / 4); the extra instructions of mix 6 are not counted.
  * Synchronises.  Allocates 8 KB of device memory (cudaMalloc) for the duration of the call and frees them.   */
 GRAY_API int gray_packed_peak(int32_t mix, int32_t iters, double* lane_ops_per_s_host, void* cuda_stream);
 

@@ -73,7 +73,7 @@ def test_argument_errors_are_reported_before_any_launch(libpath):
     assert L.gray_init_rays_polar(ctypes.byref(st), 0.5, 1000.0, 60.0, 7.5, 1.5, 10, 5, 0, None) == -2      # R_lo >= R_hi
     assert L.gray_init_rays_polar(ctypes.byref(st), 0.5, 1000.0, 60.0, 1.5, 7.5, 10, 1, 0, None) == -2      # n_theta < 2
     v = ctypes.c_double()
-    assert L.gray_packed_peak(3, 16, ctypes.byref(v), None) == -1 and L.gray_fma_peak(2, 16, ctypes.byref(v), None) == -1
+    assert L.gray_packed_peak(7, 16, ctypes.byref(v), None) == -1 and L.gray_fma_peak(2, 16, ctypes.byref(v), None) == -1
 
 
 def test_product_does_not_import_the_oracle():
