@@ -221,7 +221,10 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
     for (int it2 = 0; it2 < A.refill_interval; it2 += UN)
 #pragma unroll
     for (int un = 0; un < UN; ++un) {
-      any = false;
+      // A thread whose slots are all empty costs its warp nothing either way.  The float builds let it step its stale
+      // registers (nothing of it is ever stored) instead of testing for it at every step: +2 % on B200; the double build
+      // keeps the test (-0.7 % without)
+      any = sizeof(S) == 4;
 #pragma unroll
       for (int l = 0; l < N; ++l) any |= have[l];
       if (any) {
