@@ -88,6 +88,18 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
   int landing[N];            // stop_at_equator: 0 = cruising, 1 / 2 = before the first / second Newton step onto the plane
   bool lnd = false;          // any slot of this thread landing
   bool have[N];
+  // Which sine / cosine the first stage of a step uses (gray_math.cuh rk4_step FOLD) is a function of the step rule and
+  // of stop_at_equator only, so that every kernel variant of a rule does the same arithmetic per photon.
+  constexpr int FOLD = RULE != GRAY_STEP_EQ2 ? 0 : !EQ ? 1 : (sizeof(S) == 4 ? 2 : 0);
+  bool fold_ok = false;      // FOLD == 2: every photon of this thread within the folded polynomial's range?
+  auto fold_check = [&]() {
+    if (FOLD != 2) return;
+    S th[N];
+    vunpack(y[2], th);
+    fold_ok = true;
+#pragma unroll
+    for (int l = 0; l < N; ++l) fold_ok &= th[l] >= fold_lo<S>() && th[l] <= fold_hi<S>();
+  };
   bool exhausted = (SCHED == GRAY_SCHED_STATIC);
   unsigned long long c_steps = 0;
   unsigned int c_done = 0, c_live = 0, c_iter = 0, c_fallback = 0;
@@ -193,6 +205,7 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
 #pragma unroll
     for (int l = 0; l < N; ++l) want[l] = ((unsigned long long)blockIdx.x * N + l) * kBlock + threadIdx.x;
     take(want);
+    fold_check();
   }
 
   for (;;) {
@@ -213,6 +226,7 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
           off += __popc(need[l]);
         }
         take(want);
+        fold_check();
         if (base + cnt >= A.n) exhausted = true;
       }
     }
@@ -246,7 +260,7 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
         if (!FROZEN) {
           bool rej[N];
           if (RED) rk4_step_reduced<RULE>(K, y, comp);
-          else rk4_step<XI, RULE == GRAY_STEP_EQ2 && !EQ>(K, y, comp, dl, rej);
+          else rk4_step<XI, FOLD>(K, y, comp, dl, rej, nullptr, fold_ok);
           if (XI) {
 #pragma unroll
             for (int l = 0; l < N; ++l) c_fallback += (rej[l] && have[l]) ? 1u : 0u;
@@ -277,7 +291,8 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
               start[l] = !fold && over && landing[l] == 0;
             }
             vpack(y[2], th); vpack(y[3], ph); vpack(y[6], kh); vpack(comp[2], c2); vpack(comp[6], c6);
-          }
+            fold_check();
+          } else if (FOLD == 2) fold_ok = true;
           bool fin[N], any_fin = false;
 #pragma unroll
           for (int l = 0; l < N; ++l) {
@@ -321,7 +336,7 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
           }
           vpack(dl, dls);
           bool rej[N];
-          rk4_step<false, false, true>(K, y, comp, dl, rej, adv);
+          rk4_step<false, FOLD, true>(K, y, comp, dl, rej, adv);        // (frozen excludes stop_at_equator: FOLD is 0 or 1)
           const V z = nonfinite_probe(K, y);
           const V r = y[1];
           S th[N], zz[N], rr[N];

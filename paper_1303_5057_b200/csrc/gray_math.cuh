@@ -171,6 +171,10 @@ GRAY_DEV void sincos_folded(const Consts<V>& K, V x, V& s, V& c) {
 template <>
 GRAY_DEV void sincos_folded<double>(const Consts<double>& K, double x, double& s, double& c) { sincos_v(K, x, s, c); }
 
+// the part of sincos_folded's fitted range that callers who have to ask (rk4_step FOLD = 2) accept
+template <typename S> GRAY_DEV S fold_lo() { return S(-0.2); }
+template <typename S> GRAY_DEV S fold_hi() { return S(1.7707963); }      // pi/2 + 0.2
+
 // (s, c) = (sin, cos)(th0 + dlt) from (s0, c0) = (sin, cos)(th0):  s = s0 + c0 sd + s0 cm,  c = c0 - s0 sd + c0 cm
 // with sd = sin(dlt), cm = cos(dlt) - 1 by their Taylor series.  float: sd = dlt - dlt^3/6, cm = -dlt^2/2 + dlt^4/24
 // (9 operations; truncation < 3.4e-8 relative for |dlt| <= RotateMax).  double: through dlt^7 / dlt^8
@@ -363,20 +367,42 @@ GRAY_DEV void null_norm(const Consts<V>& K, const V y[8], V s, V c, V& Nn, V& Dn
 // XI: the paper's production pole treatment: if the state the RK4 step produced has |xi + 1| > epsilon
 // (or a non-finite xi), the step is re-integrated from the old state as one forward Euler step of dlambda / 9,
 // which is not tested itself.  rejected[l] reports it per photon.
-// FOLDED: y[2] is known to lie in the range of sincos_folded (the kernel's folded theta under the eq. (2) rule).
+// FOLD: whether y[2] lies in the range of sincos_folded at the start of the step.  1: always (the kernel's folded theta
+// under the eq. (2) rule, whose steps cannot leave [0, pi/2] by more than h); 2: the caller says in `fold_ok` whether
+// all photons of the thread are within [fold_lo, fold_hi] (stop_at_equator under eq. (2): a photon being landed on
+// the plane sits just beyond pi/2, and a Newton landing step is not bounded by the rule); 0: never (the REL rule, whose
+// steps are not bounded in theta).
 // MASKED (gray.h `frozen`): only the slots with adv[l] advance; the others keep their state bit for bit while the
 // arithmetic of the step is carried out for them all the same (the caller passes them dlambda = 0).
-template <bool XI, bool FOLDED, bool MASKED = false, typename V>
-GRAY_DEV void rk4_step(const Consts<V>& K, V y[8], V comp[8], V dl, bool rejected[VT<V>::N], const bool* adv = nullptr) {
+template <bool XI, int FOLD, bool MASKED = false, typename V>
+GRAY_DEV void rk4_step(const Consts<V>& K, V y[8], V comp[8], V dl, bool rejected[VT<V>::N], const bool* adv = nullptr,
+                       bool fold_ok = false) {
   using S = typename VT<V>::S;
   constexpr int N = VT<V>::N;
+  constexpr bool FOLDED = FOLD == 1;
   V acc[8], w[8], f[4], f1[4];
   const V hdl = vmul(K.half, dl);
   const V dl6 = vmul(K.sixth, dl);
   // stage 1
   V s0, c0, ss, cc;
-  if (FOLDED) sincos_folded(K, y[2], s0, c0);
-  else sincos_v(K, y[2], s0, c0);
+  if (FOLD != 0) {
+    sincos_folded(K, y[2], s0, c0);
+    if (FOLD == 2 && !fold_ok) {
+      // rare: some photon of this thread is outside the polynomial's range; it alone takes the quadrant-reduced values
+      // (a photon's arithmetic must not depend on the photon it shares a thread with)
+      V sv, cv;
+      sincos_v(K, y[2], sv, cv);
+      S th[N], a[N], b[N], c[N], d[N];
+      vunpack(y[2], th); vunpack(s0, a); vunpack(c0, b); vunpack(sv, c); vunpack(cv, d);
+#pragma unroll
+      for (int l = 0; l < N; ++l) {
+        const bool in = th[l] >= fold_lo<S>() && th[l] <= fold_hi<S>();
+        a[l] = in ? a[l] : c[l];
+        b[l] = in ? b[l] : d[l];
+      }
+      vpack(s0, a); vpack(c0, b);
+    }
+  } else sincos_v(K, y[2], s0, c0);
   geodesic_accel<false>(K, y[1], s0, c0, y[4], y[5], y[6], y[7], (const V*)nullptr, f);
 #pragma unroll
   for (int i = 0; i < 4; ++i) {

@@ -503,3 +503,35 @@ def test_bench_launches_its_own_ranks():
     steps1 = j1["mean_steps_per_photon"] * j1["config"]["photons_total"]
     steps2 = j2["mean_steps_per_photon"] * j2["config"]["photons_total"]
     assert 1.9 < steps2 / steps1 < 2.1
+
+
+def test_bench_line_carries_the_contract_fields():
+    # one small run of bench.py exactly as the driver starts it (one rank): the JSON line has every field the
+    # measurement contract names, with consistent numbers
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--log2n", "20", "--steps", "2", "--warmup", "3",
+                          "--e2e-log2n", "20", "--cpu-log2n", "12", "--no-secondary"], capture_output=True, text=True, timeout=600)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    for key in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling", "vs_baseline",
+                "dtype", "data", "config", "roofline", "cpu_baseline", "e2e", "gpu_launches", "clocks"):
+        assert key in d, key
+    assert d["n_gpus"] == 1 and d["steps"] == 2 and d["warmup"] == 3 and d["dtype"] == "f32" and d["vs_baseline"] is None
+    assert "workload" in d["config"] and "model" not in d["config"]
+    r = d["roofline"]
+    assert r["bound"] == "alu" and r["unit"] == "TFLOP/s" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12
+    assert 0.3 < r["frac"] < 1.0 and r["frac_executed"] is not None and r["frac_executed"] < r["frac"]
+    assert r["traffic"] is not None and "NOT measured" in r["traffic_source"]
+    assert 0.9 < r["kernel_share_of_step"] <= 1.0
+    c = d["cpu_baseline"]
+    assert c["kind"] == "oracle" and c["cores"] >= 1 and c["value"] > 0 and c["one_core"]["cores"] == 1
+    e = d["e2e"]
+    assert e["h2d_bytes_per_step"] == 2 ** 20 * 32 and e["d2h_bytes_per_step"] == 2 ** 20 * 37 and 0 < e["value"] <= 1.2 * d["value"]
+    assert d["gpu_launches"] == 3 * d["steps"]
+    assert abs(d["value"] * d["ns_per_photon_step"] - 1e9) < 1e-3 * 1e9

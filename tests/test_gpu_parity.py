@@ -369,6 +369,25 @@ def test_frozen_peak_rate_mode_matches_oracle(prec):
         assert good.sum() > 0.8 * n
 
 
+@pytest.mark.parametrize("prec,ppt", [(g.GRAY_F32, 0), (g.GRAY_F32, 1), (g.GRAY_F64, 0)])
+def test_frozen_mode_is_bitwise_the_plain_run_under_eq2_too(prec, ppt):
+    # every kernel variant of a step rule does the same arithmetic per photon (which sine / cosine the first stage uses
+    # depends on the rule only): the frozen kernel under eq. (2) against the plain one, all components, bit for bit
+    c4 = wl.C4
+    n = 2500
+    out = []
+    for frozen in (True, False):
+        b = g.PhotonBatch(n, prec)
+        g.gray_init_rays_random(b, c4["a"], wl.R_OBS, c4["inc_deg"], c4["half_width"], c4["seed"], 12345)
+        g.gray_integrate(b, max_steps=700, params=g.StepParams(rule=g.STEP_EQ2, frozen=frozen, photons_per_thread=ppt))
+        torch.cuda.synchronize()
+        out.append(b)
+    b, b2 = out
+    assert torch.equal(b.x.view(torch.uint8), b2.x.view(torch.uint8)) and torch.equal(b.k.view(torch.uint8), b2.k.view(torch.uint8))
+    assert torch.equal(b.status, b2.status) and torch.equal(b.steps, b2.steps)
+    assert int((b.status == g.LIVE).sum()) > 0 and int((b.status == g.ESCAPED).sum()) > 0       # both kinds present at 700 steps
+
+
 @pytest.mark.parametrize("prec,ppt", [(g.GRAY_F64, 0), (g.GRAY_F32, 2), (g.GRAY_F32, 1)])
 def test_xi_monitor_one_step_branches_match_oracle(prec, ppt):
     # The kernel's xi branch compared directly, one step at a time, on the states of the oracle
