@@ -159,6 +159,42 @@ def test_integrate_f32_matches_fp64_oracle(a, inc, W, nx, ny):
     assert rel_err_final(y[ok & pole], yref[ok & pole]).max() <= 1e-3
 
 
+@pytest.mark.parametrize("prec", [g.GRAY_F32, g.GRAY_F64])
+@pytest.mark.parametrize("h,r_obs,a,inc", [(1.0 / 8, 1000.0, 0.9, 60.0),      # coarse steps: stage offsets up to h = 0.125, beyond the
+                                                                            # angle-addition range -> per-photon library sincos
+                                           (1.0 / 64, 200.0, 0.5, 30.0),     # fine steps, near observer
+                                           (1.0 / 5, 1000.0, 0.99, 80.0)])   # h / 2 beyond the range too: stage 2 is tested as well
+def test_integrate_other_step_parameters_match_oracle(prec, h, r_obs, a, inc):
+    # the kernel's shortcuts are tied to h (the stage-2 angle offset is not range-tested while h / 2 is inside the
+    # rotation's range, the others fall back to a library sincos per photon when they leave it): same protocol as above
+    # at step parameters and an observer distance the configs do not use
+    W, nx, ny = 9.0, 48, 48
+    f32 = prec == g.GRAY_F32
+    b = g.PhotonBatch(nx * ny, prec)
+    g.gray_init_rays(b, a, r_obs, inc, W, nx, ny)
+    g.gray_integrate(b, max_steps=wl.MAX_STEPS, params=g.StepParams(rule=g.STEP_EQ2, h=h))
+    y, st, n = gpu_state(b)
+    ref = o.trace(a, r_obs, inc, W, nx, ny, h=h, rule=o.STEP_EQ2, init_f32=f32, threads=8)
+    al, be = grid_pixels(W, nx, ny)
+    band = edge_band(a, inc, al, be, width=0.01 if h < 0.1 else 0.03)        # coarse steps blur the critical curve itself
+    mism = st != ref["status"]
+    assert mism.mean() <= 2e-3 and np.all(band[mism]), (mism.sum(), np.sum(mism & ~band))
+    assert not np.any(st == g.LIVE)
+    diff = np.flatnonzero((n != ref["steps"]) & ~mism)
+    assert diff.size <= 0.01 * n.size
+    yref = ref["y"].copy()
+    if diff.size:
+        yref[diff] = o.trace(a, r_obs, inc, W, nx, ny, idx=diff.astype(np.uint64), h=h, rule=o.STEP_EQ2, init_f32=f32,
+                             force_steps=n[diff])["y"]
+    ok = ~band & ~mism & (ref["status"] != o.BAD)
+    assert ok.mean() > 0.9
+    err = rel_err_final(y[ok], yref[ok])
+    if f32:
+        assert np.quantile(err, 0.99) <= 2e-5 and err.max() <= 1e-3, (np.quantile(err, 0.99), err.max())
+    else:
+        assert err.max() <= 1e-9, err.max()
+
+
 # What the fp32 range allows: a state with a component beyond ~1e9 has fourth powers (Sigma^2) beyond 3e38
 FP32_RANGE = 1e9
 
