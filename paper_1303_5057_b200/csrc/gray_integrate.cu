@@ -89,16 +89,18 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
   bool lnd = false;          // any slot of this thread landing
   bool have[N];
   // Which sine / cosine the first stage of a step uses (gray_math.cuh rk4_step FOLD) is a function of the step rule and
-  // of stop_at_equator only, so that every kernel variant of a rule does the same arithmetic per photon.
-  constexpr int FOLD = RULE != GRAY_STEP_EQ2 ? 0 : !EQ ? 1 : (sizeof(S) == 4 ? 2 : 0);
-  bool fold_ok = false;      // FOLD == 2: every photon of this thread within the folded polynomial's range?
-  auto fold_check = [&]() {
+  // of stop_at_equator only, so that every kernel variant of a rule does the same arithmetic per photon: under eq. (2)
+  // without landing steps the folded polynomial always (1); otherwise (REL steps are not bounded in theta, landing steps
+  // sit beyond pi/2) the polynomial for every photon within its range, photon by photon (2; float builds).
+  constexpr int FOLD = (RULE == GRAY_STEP_EQ2 && !EQ) ? 1 : (sizeof(S) == 4 ? 2 : 0);
+  bool fold_ok = false;      // FOLD == 2: every photon this thread is advancing within the folded polynomial's range?
+  auto fold_check = [&](const bool use[N]) {
     if (FOLD != 2) return;
     S th[N];
     vunpack(y[2], th);
     fold_ok = true;
 #pragma unroll
-    for (int l = 0; l < N; ++l) fold_ok &= th[l] >= fold_lo<S>() && th[l] <= fold_hi<S>();
+    for (int l = 0; l < N; ++l) fold_ok &= !use[l] || (th[l] >= fold_lo<S>() && th[l] <= fold_hi<S>());
   };
   bool exhausted = (SCHED == GRAY_SCHED_STATIC);
   unsigned long long c_steps = 0;
@@ -205,7 +207,7 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
 #pragma unroll
     for (int l = 0; l < N; ++l) want[l] = ((unsigned long long)blockIdx.x * N + l) * kBlock + threadIdx.x;
     take(want);
-    fold_check();
+    fold_check(have);
   }
 
   for (;;) {
@@ -226,7 +228,7 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
           off += __popc(need[l]);
         }
         take(want);
-        fold_check();
+        fold_check(have);
         if (base + cnt >= A.n) exhausted = true;
       }
     }
@@ -291,7 +293,7 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
               start[l] = !fold && over && landing[l] == 0;
             }
             vpack(y[2], th); vpack(y[3], ph); vpack(y[6], kh); vpack(comp[2], c2); vpack(comp[6], c6);
-            fold_check();
+            fold_check(have);
           } else if (FOLD == 2) fold_ok = true;
           bool fin[N], any_fin = false;
 #pragma unroll
@@ -336,7 +338,7 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
           }
           vpack(dl, dls);
           bool rej[N];
-          rk4_step<false, FOLD, true>(K, y, comp, dl, rej, adv);        // (frozen excludes stop_at_equator: FOLD is 0 or 1)
+          rk4_step<false, FOLD, true>(K, y, comp, dl, rej, adv, fold_ok);
           const V z = nonfinite_probe(K, y);
           const V r = y[1];
           S th[N], zz[N], rr[N];
@@ -351,7 +353,8 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
             for (int l = 0; l < N; ++l)
               if (adv[l]) remap_theta(th[l], ph[l], kh[l], c2[l], c6[l], mirrored[l], true);
             vpack(y[2], th); vpack(y[3], ph); vpack(y[6], kh); vpack(comp[2], c2); vpack(comp[6], c6);
-          }
+            fold_check(adv);
+          } else if (FOLD == 2) fold_ok = true;            // every advancing photon is inside [0, pi/2]; the others do not matter
 #pragma unroll
           for (int l = 0; l < N; ++l) {
             if (have[l]) {
