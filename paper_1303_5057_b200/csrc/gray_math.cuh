@@ -27,10 +27,12 @@
 #include "gray_vec.cuh"
 
 // Components of y = (t, d, th, phi, k^t, k^r, k^th, k^phi) whose update is a compensated sum in the float builds
-// (bit i = component i).  t (bit 0) is left out: it feeds nothing back, and measured on B200 the final (r, theta, phi)
-// and the drift of E, L_z, Q are bit-for-bit the same with and without it.
+// (bit i = component i).  t (bit 0) and phi (bit 3) are left out: the metric depends on neither, so they feed nothing
+// back.  Measured on B200: with or without t the final (r, theta, phi) and the drift of E, L_z, Q
+// are bit-for-bit the same; without phi the error of the final state against the oracle is unchanged at the 99th
+// percentile and at the maximum (phi's own rounding, ~ 1e-7 per step, stays far below the error r and theta carry).
 #ifndef GRAY_COMP_MASK
-#define GRAY_COMP_MASK 0xfe
+#define GRAY_COMP_MASK 0xf6
 #endif
 
 namespace gray {
