@@ -46,9 +46,10 @@ def parse():
                     "the north star's 2^30; lowered, and said so in config.workload, if the device lacks the 40 GB it needs)")
     ap.add_argument("--prec", default="f32", choices=["f32", "f64"])
     ap.add_argument("--rule", default="eq2", choices=["eq2", "rel"])
-    ap.add_argument("--case", default="realistic", choices=["realistic", "peak", "projection"],
+    ap.add_argument("--case", default="realistic", choices=["realistic", "peak", "projection", "ring"],
                     help="projection = the paper's first benchmark (P:130-140, Fig. 4): run time of the grid projection "
-                         "onto the equatorial plane (a = 0.95, i = 60 deg) against the number of rays")
+                         "onto the equatorial plane (a = 0.95, i = 60 deg) against the number of rays; ring = the paper's "
+                         "photon-ring study (section 4, P:165-210): 16 spins x 19 inclinations x 6000 x 181 rays")
     ap.add_argument("--schedule", default="refill", choices=["refill", "static"])
     ap.add_argument("--refill-interval", type=int, default=0)
     ap.add_argument("--photons-per-thread", type=int, default=0, help="0 = library default (2 for f32: packed FFMA2), 1, 2")
@@ -551,6 +552,62 @@ def run_projection(args):
     print(json.dumps(out), flush=True)
 
 
+def run_ring(args):
+    """Paper section 4: the photon ring of a Kerr black hole for 16 spins a_j = 1 - 10^(-j/5) and 19
+    inclinations 0, 5, ..., 90 deg, each image a polar grid of 6000 x 181 rays over (1.5 M, 7.5 M) x [0, pi] at
+    r_obs = 1000 M (3.3e8 geodesics), with the xi monitor on as in the paper: init -> integrate -> ring statistics
+    (D, <R>, A of eqs. 6-8) per case.  Timed with CUDA events over the whole study; tests/test_gpu_configs.py compares every
+    case with the closed-form Bardeen curve and the oracle."""
+    import torch
+
+    import paper_1303_5057_b200 as g
+    from paper_1303_5057_b200 import workloads as wl
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    R_lo, R_hi, n_R, n_th = 1.5, 7.5, 6000, 181
+    b = g.PhotonBatch(n_R * n_th, g.GRAY_F32)
+    params = g.StepParams(rule=g.STEP_EQ2, xi_epsilon=1e-3)
+    show = {(0, 0), (0, 60), (5, 60), (10, 30), (10, 60), (10, 90), (15, 0), (15, 60), (15, 90)}
+    rows, steps, fallback, lost = [], 0, 0, 0
+
+    def study(record):
+        nonlocal steps, fallback, lost
+        for j in range(16):
+            a = 1.0 - 10.0 ** (-j / 5.0)
+            for inc in range(0, 91, 5):
+                g.gray_init_rays_polar(b, a, wl.R_OBS, float(inc), R_lo, R_hi, n_R, n_th)
+                g.gray_integrate(b, max_steps=wl.MAX_STEPS, params=params)
+                s = g.gray_ring_polar(b, None, bridge_axis=True)           # synchronises: the case's result on the host
+                if record:
+                    c = g.gray_integrate_counters(b)
+                    steps += c["photon_steps"]
+                    fallback += c["fallback_steps"]
+                    lost += s["axis_rays_lost"]
+                    if (j, inc) in show:
+                        rows.append({"a": round(a, 6), "inc_deg": inc, "D": s["D"], "R_mean": s["R_mean"], "A": s["A"],
+                                     "alpha_min": s["alpha_min"], "alpha_max": s["alpha_max"]})
+
+    study(False)                                                           # warm-up pass
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    study(True)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    n_geo = 16 * 19 * n_R * n_th
+    out = {"metric": "run time of the paper's photon-ring study (section 4)", "unit": "s", "value": ms * 1e-3, "n_gpus": 1,
+           "higher_is_better": False, "data": "synthetic", "dtype": "f32",
+           "config": {"workload": "304 images (16 spins a_j = 1 - 10^(-j/5) x 19 inclinations 0..90 deg), polar grid 6000 x 181 rays over "
+                                  "(1.5, 7.5) M x [0, pi] at r_obs = 1000 M, eq. (2) rule h = 1/32, xi monitor eps = 1e-3",
+                      "timer": "CUDA events around the whole study (init + integrate + ring statistics read back per case), after one warm-up pass"},
+           "geodesics": n_geo, "geodesics_per_s": n_geo / (ms * 1e-3), "photon_steps": steps, "photon_steps_per_s": steps / (ms * 1e-3),
+           "xi_fallback_steps": fallback, "axis_rays_lost": lost, "rows": rows,
+           "paper_context": "16 x 19 x 6000 x 181 ~ 3e8 geodesics, 'none of them fails at the pole' (P:109, P:170); ring radius ~ 5.2 M, "
+                            "nearly circular up to a ~ 0.9 (P:172-174)"}
+    print(json.dumps(out), flush=True)
+
+
 def launcher_command(args, argv, port=None):
     """`python bench.py --gpus N` started by hand (no torchrun environment): the command that re-runs this script as N
     ranks on this node, one per GPU, the way the driver launches it.  None if no re-launch is needed."""
@@ -574,6 +631,9 @@ def main():
         raise SystemExit(subprocess.call(cmd, env=env))
     if args.case == "projection" and args.impl != "reference":
         run_projection(args)
+        return
+    if args.case == "ring" and args.impl != "reference":
+        run_ring(args)
         return
     if args.impl == "reference":
         run_reference(args)
