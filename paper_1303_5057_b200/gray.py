@@ -142,6 +142,27 @@ class PhotonBatch:
         self.c.nx, self.c.ny, self.c.seed, self.c.p0, self.c.pixels = nx, ny, seed, p0, pixels
 
 
+def _slice(self, lo, hi):
+    """A batch over photons lo .. hi-1 of this one, sharing its buffers (its own workspace and image-plane fields): several
+    images that differ only in what gray_integrate does not read (inclination, pixel grid) can be initialised slice by slice,
+    integrated in ONE launch over the parent batch, and evaluated slice by slice."""
+    lo, hi = int(lo), int(hi)
+    if not 0 <= lo <= hi <= self.n:
+        raise GrayError("slice out of range")
+    v = object.__new__(PhotonBatch)
+    v.n, v.prec = hi - lo, self.prec
+    v.x, v.k, v.status, v.steps = self.x[lo:hi], self.k[lo:hi], self.status[lo:hi], self.steps[lo:hi]
+    v.workspace = torch.zeros_like(self.workspace)
+    v.resume = self.resume[lo:hi] if self.resume is not None else None
+    v.c = _State(v.x.data_ptr(), v.k.data_ptr(), v.status.data_ptr(), v.steps.data_ptr(), v.n, v.prec, self.c.pixels,
+                 self.c.a, self.c.r_obs, self.c.inc_deg, self.c.half_width, self.c.nx, self.c.ny, self.c.seed, self.c.p0 + lo,
+                 self.c.r_lo, v.resume.data_ptr() if v.resume is not None else None)
+    return v
+
+
+PhotonBatch.slice = _slice
+
+
 def gray_workspace_bytes(n):
     return int(lib().gray_workspace_bytes(int(n)))
 

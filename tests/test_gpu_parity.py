@@ -572,6 +572,35 @@ def test_integrate_host_matches_device_path():
         assert cnt["photon_steps"] == cnt_dev["photon_steps"] and cnt["photons_done"] == n
 
 
+def test_batch_slices_share_one_launch():
+    # images that differ only in what gray_integrate does not read (inclination, grid) initialised slice by slice and
+    # integrated in ONE launch over the parent batch: bit for bit the per-image runs, and the per-slice evaluation agrees
+    a, R_lo, R_hi, n_R, n_th = 0.9, 1.5, 7.5, 300, 31
+    n = n_R * n_th
+    incs = (10.0, 60.0, 85.0)
+    big = g.PhotonBatch(n * len(incs), g.GRAY_F32)
+    views = [big.slice(i * n, (i + 1) * n) for i in range(len(incs))]
+    p = g.StepParams(rule=g.STEP_EQ2, xi_epsilon=1e-3)
+    for v, inc in zip(views, incs):
+        g.gray_init_rays_polar(v, a, wl.R_OBS, inc, R_lo, R_hi, n_R, n_th)
+    big.set_image_plane(a, wl.R_OBS, 0.0, R_hi)
+    g.gray_integrate(big, max_steps=wl.MAX_STEPS, params=p)
+    total = g.gray_integrate_counters(big)["photon_steps"]
+    seen = 0
+    for v, inc in zip(views, incs):
+        one = g.PhotonBatch(n, g.GRAY_F32)
+        g.gray_init_rays_polar(one, a, wl.R_OBS, inc, R_lo, R_hi, n_R, n_th)
+        g.gray_integrate(one, max_steps=wl.MAX_STEPS, params=p)
+        seen += g.gray_integrate_counters(one)["photon_steps"]
+        assert torch.equal(one.x.view(torch.uint8), v.x.view(torch.uint8)) and torch.equal(one.k.view(torch.uint8), v.k.view(torch.uint8))
+        assert torch.equal(one.status, v.status) and torch.equal(one.steps, v.steps)
+        assert g.gray_ring_polar(one, None, bridge_axis=True) == g.gray_ring_polar(v, None, bridge_axis=True)
+        assert g.gray_classify(one) == g.gray_classify(v)
+    assert seen == total
+    with pytest.raises(g.GrayError):
+        big.slice(0, big.n + 1)
+
+
 @pytest.mark.parametrize("prec", [g.GRAY_F32, g.GRAY_F64])
 def test_paper_horizon_standoff_delta(prec):
     # the paper's own termination: stop at r_bh + delta with delta ~ 1e-6 (r_capture_factor = 0); only eq. (2)'s
