@@ -46,10 +46,11 @@ def parse():
                     "the north star's 2^30; lowered, and said so in config.workload, if the device lacks the 40 GB it needs)")
     ap.add_argument("--prec", default="f32", choices=["f32", "f64"])
     ap.add_argument("--rule", default="eq2", choices=["eq2", "rel"])
-    ap.add_argument("--case", default="realistic", choices=["realistic", "peak", "projection", "ring"],
+    ap.add_argument("--case", default="realistic", choices=["realistic", "peak", "projection", "ring", "survey"],
                     help="projection = the paper's first benchmark (P:130-140, Fig. 4): run time of the grid projection "
                          "onto the equatorial plane (a = 0.95, i = 60 deg) against the number of rays; ring = the paper's "
-                         "photon-ring study (section 4, P:165-210): 16 spins x 19 inclinations x 6000 x 181 rays")
+                         "photon-ring study (section 4, P:165-210): 16 spins x 19 inclinations x 6000 x 181 rays; survey = "
+                         "BASELINE config C5: 11 spins x 9 inclinations, 1024 x 1024 images, shadow statistics per case")
     ap.add_argument("--schedule", default="refill", choices=["refill", "static"])
     ap.add_argument("--refill-interval", type=int, default=0)
     ap.add_argument("--photons-per-thread", type=int, default=0, help="0 = library default (2 for f32: packed FFMA2), 1, 2")
@@ -616,6 +617,67 @@ def run_ring(args):
     print(json.dumps(out), flush=True)
 
 
+def run_survey(args):
+    """BASELINE config C5: the shadow / photon-ring survey, spins {0, 0.1, ..., 0.9, 0.99} x inclinations {5, 15, ..., 85} deg
+    (99 cases), each a 1024 x 1024 image over +-10 M at r_obs = 1000 M, fp32, eq. (2) rule, xi monitor on; per case the
+    capture map, shadow area, centroid, D, <R>, A and the boundary radius on 360 spokes (gray_classify + gray_shadow_edge).
+    The nine images of a spin share one integrate launch (PhotonBatch.slice)."""
+    import torch
+
+    import paper_1303_5057_b200 as g
+    from paper_1303_5057_b200 import workloads as wl
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    c5 = wl.C5
+    nx, ny, W = c5["nx"], c5["ny"], c5["half_width"]
+    n_img = nx * ny
+    incs = c5["incs_deg"]
+    big = g.PhotonBatch(n_img * len(incs), g.GRAY_F32)
+    views = [big.slice(i * n_img, (i + 1) * n_img) for i in range(len(incs))]
+    cmap = torch.empty((ny, nx), dtype=torch.uint8, device="cuda")
+    radius = torch.empty((360,), dtype=torch.float64, device="cuda")
+    params = g.StepParams(rule=g.STEP_EQ2, xi_epsilon=1e-3)
+    show = {(0.0, 45.0), (0.5, 45.0), (0.9, 5.0), (0.9, 45.0), (0.9, 85.0), (0.99, 45.0), (0.99, 85.0)}
+    rows, steps, bad = [], 0, 0
+
+    def study(record):
+        nonlocal steps, bad
+        for a in c5["spins"]:
+            for v, inc in zip(views, incs):
+                g.gray_init_rays(v, a, wl.R_OBS, inc, W, nx, ny)
+            big.set_image_plane(a, wl.R_OBS, 0.0, W)
+            g.gray_integrate(big, max_steps=wl.MAX_STEPS, params=params)
+            if record:
+                steps += g.gray_integrate_counters(big)["photon_steps"]
+            for v, inc in zip(views, incs):
+                counts = g.gray_classify(v, cmap)
+                s = g.gray_shadow_edge(v, 360, radius)                     # synchronises: the image's result on the host
+                if record:
+                    bad += counts[g.BAD] + counts[g.LIVE]
+                    if (a, inc) in show:
+                        rows.append({"a": a, "inc_deg": inc, "captured": counts[g.CAPTURED], "area": s["area"],
+                                     "centroid_alpha": s["centroid_alpha"], "D": s["D"], "R_mean": s["R_mean"], "A": s["A"]})
+
+    study(False)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    study(True)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    n_geo = len(c5["spins"]) * len(incs) * n_img
+    out = {"metric": "run time of the shadow survey (BASELINE config C5)", "unit": "s", "value": ms * 1e-3, "n_gpus": 1,
+           "higher_is_better": False, "data": "synthetic", "dtype": "f32",
+           "config": {"workload": "99 images (11 spins x 9 inclinations), 1024 x 1024 pixels over +-10 M at r_obs = 1000 M, eq. (2) rule "
+                                  "h = 1/32, xi monitor eps = 1e-3, cap 20000 steps",
+                      "timer": "CUDA events around the whole survey (per spin: 9 x init, one integrate launch, 9 x (classify + shadow edge read "
+                               "back)), after one warm-up pass"},
+           "geodesics": n_geo, "geodesics_per_s": n_geo / (ms * 1e-3), "photon_steps": steps, "photon_steps_per_s": steps / (ms * 1e-3),
+           "rays_bad_or_live": bad, "rows": rows}
+    print(json.dumps(out), flush=True)
+
+
 def launcher_command(args, argv, port=None):
     """`python bench.py --gpus N` started by hand (no torchrun environment): the command that re-runs this script as N
     ranks on this node, one per GPU, the way the driver launches it.  None if no re-launch is needed."""
@@ -642,6 +704,9 @@ def main():
         return
     if args.case == "ring" and args.impl != "reference":
         run_ring(args)
+        return
+    if args.case == "survey" and args.impl != "reference":
+        run_survey(args)
         return
     if args.impl == "reference":
         run_reference(args)
