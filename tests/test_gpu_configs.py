@@ -535,3 +535,20 @@ def test_bench_line_carries_the_contract_fields():
     assert e["h2d_bytes_per_step"] == 2 ** 20 * 32 and e["d2h_bytes_per_step"] == 2 ** 20 * 37 and 0 < e["value"] <= 1.2 * d["value"]
     assert d["gpu_launches"] == 3 * d["steps"]
     assert abs(d["value"] * d["ns_per_photon_step"] - 1e9) < 1e-3 * 1e9
+
+
+def test_bench_survey_case_runs_and_reproduces_the_schwarzschild_disc():
+    # bench.py --case survey (BASELINE config C5 as a timed application, nine images of a spin per launch): one JSON line,
+    # no ray lost with the xi monitor on, and the a = 0 image is the disc of radius sqrt(27)
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--case", "survey"], capture_output=True, text=True, timeout=600)
+    assert out.returncode == 0, out.stderr[-2000:]
+    d = json.loads([l for l in out.stdout.splitlines() if l.startswith("{")][0])
+    assert d["geodesics"] == 99 * 1024 * 1024 and d["rays_bad_or_live"] == 0 and d["value"] > 0
+    r0 = [r for r in d["rows"] if r["a"] == 0.0][0]
+    assert abs(r0["area"] - 27 * np.pi) < 0.1 and abs(r0["R_mean"] - np.sqrt(27)) < 0.01 and abs(r0["D"]) < 0.02
+    assert all(r["D"] > 0 for r in d["rows"] if r["a"] > 0)           # the shadow is displaced towards +alpha for a > 0 (R2)
