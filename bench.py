@@ -499,6 +499,13 @@ def run_gray(args):
         out["e2e"] = e2e
     if secondary:
         out["secondary"] = secondary
+    if not args.no_secondary and world == 1:
+        # the applications this repository quotes, in the same run: BASELINE config C5 and the paper's photon-ring study
+        apps = []
+        for fn in (run_survey, run_ring):
+            a = fn(args, emit=False)
+            apps.append({k: a[k] for k in ("metric", "value", "unit", "geodesics", "geodesics_per_s", "photon_steps", "photon_steps_per_s", "config")})
+        out["applications"] = apps
     if not args.no_cpu_baseline:
         import oracle as o                          # cpu_baseline leg only
         threads = max(1, o.hardware_threads())
@@ -553,7 +560,7 @@ def run_projection(args):
     print(json.dumps(out), flush=True)
 
 
-def run_ring(args):
+def run_ring(args, emit=True):
     """Paper section 4: the photon ring of a Kerr black hole for 16 spins a_j = 1 - 10^(-j/5) and 19
     inclinations 0, 5, ..., 90 deg, each image a polar grid of 6000 x 181 rays over (1.5 M, 7.5 M) x [0, pi] at
     r_obs = 1000 M (3.3e8 geodesics), with the xi monitor on as in the paper: init -> integrate -> ring statistics
@@ -614,10 +621,13 @@ def run_ring(args):
            "xi_fallback_steps": fallback, "axis_rays_lost": lost, "rows": rows,
            "paper_context": "16 x 19 x 6000 x 181 ~ 3e8 geodesics, 'none of them fails at the pole' (P:109, P:170); ring radius ~ 5.2 M, "
                             "nearly circular up to a ~ 0.9 (P:172-174)"}
-    print(json.dumps(out), flush=True)
+    del big, views
+    if emit:
+        print(json.dumps(out), flush=True)
+    return out
 
 
-def run_survey(args):
+def run_survey(args, emit=True):
     """BASELINE config C5: the shadow / photon-ring survey, spins {0, 0.1, ..., 0.9, 0.99} x inclinations {5, 15, ..., 85} deg
     (99 cases), each a 1024 x 1024 image over +-10 M at r_obs = 1000 M, fp32, eq. (2) rule, xi monitor on; per case the
     capture map, shadow area, centroid, D, <R>, A and the boundary radius on 360 spokes (gray_classify + gray_shadow_edge).
@@ -675,7 +685,10 @@ def run_survey(args):
                                "back)), after one warm-up pass"},
            "geodesics": n_geo, "geodesics_per_s": n_geo / (ms * 1e-3), "photon_steps": steps, "photon_steps_per_s": steps / (ms * 1e-3),
            "rays_bad_or_live": bad, "rows": rows}
-    print(json.dumps(out), flush=True)
+    del big, views
+    if emit:
+        print(json.dumps(out), flush=True)
+    return out
 
 
 def launcher_command(args, argv, port=None):
