@@ -83,14 +83,24 @@ struct EdgeArgs {
 
 // rho(vartheta): march outwards from the image origin in half-pixel steps until the pixel under the
 // sample is not captured (or the image ends); the edge is the mid-point of the last two samples.
-__device__ double spoke_radius(const EdgeArgs& A, double da, double db, double delta, double cv, double sv) {
-  for (long long j = 0;; ++j) {
+// One warp per spoke: its lanes look at 32 consecutive samples at a time and the first one that stops the march is
+// found by ballot (the samples do not depend on each other, only the stopping rule does).
+constexpr int kMaxSpokesInShared = 5120;        // radii of up to this many spokes are kept in shared memory (40 KB)
+__device__ double spoke_radius_warp(const EdgeArgs& A, double da, double db, double delta, double cv, double sv) {
+  const int lane = threadIdx.x & 31;
+  for (long long j0 = 0;; j0 += 32) {
+    const long long j = j0 + lane;
     const double q = (double)j * delta;
     const long long col = (long long)floor((q * cv + A.W) / da);
     const long long row = (long long)floor((q * sv + A.W) / db);
     const bool inside = col >= 0 && col < A.nx && row >= 0 && row < A.ny;
-    if (!inside) return ((double)j - 0.5) * delta;
-    if (A.status[row * A.nx + col] != GRAY_CAPTURED) return j == 0 ? 0.0 : ((double)j - 0.5) * delta;
+    const bool stop = !inside || A.status[row * A.nx + col] != GRAY_CAPTURED;
+    const unsigned m = __ballot_sync(0xffffffffu, stop);
+    if (m) {
+      const long long js = j0 + (__ffs(m) - 1);
+      const bool in_s = (__ballot_sync(0xffffffffu, inside) >> (__ffs(m) - 1)) & 1u;
+      return (!in_s || js > 0) ? ((double)js - 0.5) * delta : 0.0;
+    }
   }
 }
 
@@ -105,9 +115,10 @@ __device__ double block_sum(double v, double* sh) {
   return t;
 }
 
-// one block: spokes, then eqs. (6)-(8)
+// one block: spokes (a warp each), then eqs. (6)-(8)
 __global__ void __launch_bounds__(1024) shadow_edge_kernel(const __grid_constant__ EdgeArgs A) {
   __shared__ double sh[32];
+  __shared__ double rho_sh[kMaxSpokesInShared];
   Workspace* ws = A.ws;
   const double da = 2.0 * A.W / (double)A.nx, db = 2.0 * A.W / (double)A.ny;
   const double delta = fmin(da, db) / 2.0;
@@ -116,26 +127,38 @@ __global__ void __launch_bounds__(1024) shadow_edge_kernel(const __grid_constant
   const double amax = ncap ? -A.W + (double)(ws->max_col + 1) * da : 0.0;
   const double centre = (amin + amax) / 2.0;
   const double two_pi = 2.0 * 3.14159265358979323846;
+  const int warp = threadIdx.x >> 5, n_warps = blockDim.x >> 5, lane = threadIdx.x & 31;
+  // R_k = distance of the edge point on spoke k from the ring's centre; the spoke's rho from shared memory if it is there
+  auto R_of = [&](int k, double rho) {
+    const double vt = two_pi * ((double)k + 0.5) / (double)A.n_angles;
+    double sv, cv;
+    sincos(vt, &sv, &cv);
+    const double x = rho * cv - centre, y = rho * sv;
+    return sqrt(x * x + y * y);
+  };
+  auto rho_of = [&](int k) {                       // called by whole warps
+    const double vt = two_pi * ((double)k + 0.5) / (double)A.n_angles;
+    double sv, cv;
+    sincos(vt, &sv, &cv);
+    return spoke_radius_warp(A, da, db, delta, cv, sv);
+  };
   double sumR = 0.0;
-  for (int k = threadIdx.x; k < A.n_angles; k += blockDim.x) {
-    const double vt = two_pi * ((double)k + 0.5) / (double)A.n_angles;
-    double sv, cv;
-    sincos(vt, &sv, &cv);
-    const double rho = spoke_radius(A, da, db, delta, cv, sv);
-    if (A.radius) A.radius[k] = rho;
-    const double x = rho * cv - centre, y = rho * sv;
-    sumR += sqrt(x * x + y * y);
+  for (int k = warp; k < A.n_angles; k += n_warps) {
+    const double rho = rho_of(k);
+    if (lane == 0) {
+      if (k < kMaxSpokesInShared) rho_sh[k] = rho;
+      if (A.radius) A.radius[k] = rho;
+      sumR += R_of(k, rho);
+    }
   }
-  const double mean = A.n_angles > 0 ? block_sum(sumR, sh) / (double)A.n_angles : 0.0;
+  const double mean = A.n_angles > 0 ? block_sum(sumR, sh) / (double)A.n_angles : 0.0;     // (block_sum synchronises)
   double var = 0.0;
-  for (int k = threadIdx.x; k < A.n_angles; k += blockDim.x) {
-    const double vt = two_pi * ((double)k + 0.5) / (double)A.n_angles;
-    double sv, cv;
-    sincos(vt, &sv, &cv);
-    const double rho = spoke_radius(A, da, db, delta, cv, sv);
-    const double x = rho * cv - centre, y = rho * sv;
-    const double d = sqrt(x * x + y * y) - mean;
-    var += d * d;
+  for (int k = warp; k < A.n_angles; k += n_warps) {
+    const double rho = k < kMaxSpokesInShared ? rho_sh[k] : rho_of(k);
+    if (lane == 0) {
+      const double d = R_of(k, rho) - mean;
+      var += d * d;
+    }
   }
   var = A.n_angles > 0 ? block_sum(var, sh) / (double)A.n_angles : 0.0;
   if (threadIdx.x == 0) {
@@ -150,8 +173,8 @@ __global__ void __launch_bounds__(1024) shadow_edge_kernel(const __grid_constant
   }
 }
 
-// Photon ring on the paper's polar grid (gray_ring_polar in gray.h; eqs. 6-10).  One block; a thread
-// per spoke walks inwards to the outermost captured cell, then eqs. (6)-(8) by block reductions (trapezoidal rule).
+// Photon ring on the paper's polar grid (gray_ring_polar in gray.h; eqs. 6-10).  One block; a warp per
+// spoke finds the outermost captured cell, then eqs. (6)-(8) by block reductions (trapezoidal rule).
 struct RingArgs {
   const uint8_t* status;
   long long n_R, n_theta;
@@ -161,46 +184,66 @@ struct RingArgs {
   Workspace* ws;
 };
 
-__device__ double ring_radius_raw(const RingArgs& A, long long k) {
+// outer edge of the outermost captured cell of spoke k, by a whole warp: the lanes share the cells, the largest captured
+// index wins
+__device__ double ring_radius_raw_warp(const RingArgs& A, long long k) {
   const uint8_t* row = A.status + k * A.n_R;
-  long long j = A.n_R;
-  while (j > 0 && row[j - 1] != GRAY_CAPTURED) --j;      // outer edge of the outermost captured cell
-  return A.R_lo + (double)j * ((A.R_hi - A.R_lo) / (double)A.n_R);
-}
-__device__ double ring_radius(const RingArgs& A, long long k) {
-  if (A.bridge_axis && A.n_theta >= 3 && (A.n_theta % 2) == 1 && k == (A.n_theta - 1) / 2)
-    return 0.5 * (ring_radius_raw(A, k - 1) + ring_radius_raw(A, k + 1));      // the axis spoke (gray.h)
-  return ring_radius_raw(A, k);
+  long long best = 0;
+  for (long long j = threadIdx.x & 31; j < A.n_R; j += 32)
+    if (row[j] == GRAY_CAPTURED) best = j + 1;
+  for (int o = 16; o > 0; o >>= 1) {
+    const long long other = __shfl_xor_sync(0xffffffffu, best, o);
+    best = other > best ? other : best;
+  }
+  return A.R_lo + (double)best * ((A.R_hi - A.R_lo) / (double)A.n_R);
 }
 
 __global__ void __launch_bounds__(1024) ring_polar_kernel(const __grid_constant__ RingArgs A) {
   __shared__ double sh[32];
+  __shared__ double raw_sh[kMaxSpokesInShared];
   const double pi = 3.14159265358979323846;
-  const double amax = ring_radius(A, 0), amin = -ring_radius(A, A.n_theta - 1);
+  const int warp = threadIdx.x >> 5, n_warps = blockDim.x >> 5, lane = threadIdx.x & 31;
+  const long long mid = (A.n_theta - 1) / 2;
+  const bool has_axis = A.n_theta >= 3 && (A.n_theta % 2) == 1;
+  for (long long k = warp; k < A.n_theta && k < kMaxSpokesInShared; k += n_warps) {
+    const double r = ring_radius_raw_warp(A, k);
+    if (lane == 0) raw_sh[k] = r;
+  }
+  __syncthreads();
+  auto raw_of = [&](long long k) { return k < kMaxSpokesInShared ? raw_sh[k] : ring_radius_raw_warp(A, k); };   // whole warps
+  auto radius_of = [&](long long k) {
+    if (A.bridge_axis && has_axis && k == mid) return 0.5 * (raw_of(k - 1) + raw_of(k + 1));      // the axis spoke (gray.h)
+    return raw_of(k);
+  };
+  const double amax = radius_of(0), amin = -radius_of(A.n_theta - 1);
   const double centre = (amin + amax) / 2.0;
   const double step = pi / (double)(A.n_theta - 1);
-  auto R_of = [&](long long k, bool store) {
-    const double rho = ring_radius(A, k);
-    if (store && A.radius) A.radius[k] = rho;
+  auto R_of = [&](long long k, double rho) {
     double sv, cv;
     sincos((double)k * step, &sv, &cv);
     const double x = rho * cv - centre, y = rho * sv;
     return sqrt(x * x + y * y);
   };
   double sum = 0.0;
-  for (long long k = threadIdx.x; k < A.n_theta; k += blockDim.x)
-    sum += ((k == 0 || k == A.n_theta - 1) ? 0.5 : 1.0) * R_of(k, true);
+  for (long long k = warp; k < A.n_theta; k += n_warps) {
+    const double rho = radius_of(k);
+    if (lane == 0) {
+      if (A.radius) A.radius[k] = rho;
+      sum += ((k == 0 || k == A.n_theta - 1) ? 0.5 : 1.0) * R_of(k, rho);
+    }
+  }
   const double mean = block_sum(sum, sh) / (double)(A.n_theta - 1);
   double var = 0.0;
-  for (long long k = threadIdx.x; k < A.n_theta; k += blockDim.x) {
-    const double d = R_of(k, false) - mean;
-    var += ((k == 0 || k == A.n_theta - 1) ? 0.5 : 1.0) * d * d;
+  for (long long k = warp; k < A.n_theta; k += n_warps) {
+    const double rho = radius_of(k);
+    if (lane == 0) {
+      const double d = R_of(k, rho) - mean;
+      var += ((k == 0 || k == A.n_theta - 1) ? 0.5 : 1.0) * d * d;
+    }
   }
   var = block_sum(var, sh) / (double)(A.n_theta - 1);
   // the axis spoke (vartheta = pi/2, n_theta odd), reported whether or not it is bridged: its radius as traced, the
   // radius used, and how many of its rays did not end CAPTURED or ESCAPED (gray.h)
-  const long long mid = (A.n_theta - 1) / 2;
-  const bool has_axis = A.n_theta >= 3 && (A.n_theta % 2) == 1;
   double lost = 0.0;
   if (has_axis)
     for (long long j = threadIdx.x; j < A.n_R; j += blockDim.x) {
@@ -208,14 +251,15 @@ __global__ void __launch_bounds__(1024) ring_polar_kernel(const __grid_constant_
       lost += (st != GRAY_CAPTURED && st != GRAY_ESCAPED) ? 1.0 : 0.0;
     }
   lost = block_sum(lost, sh);
+  const double axis_raw = has_axis ? raw_of(mid) : 0.0, axis_used = has_axis ? radius_of(mid) : 0.0;     // (every warp, uniformly)
   if (threadIdx.x == 0) {
     A.ws->stats[0] = amin;
     A.ws->stats[1] = amax;
     A.ws->stats[2] = fabs(amin + amax) / 2.0;
     A.ws->stats[3] = mean;
     A.ws->stats[4] = 2.0 * sqrt(var);
-    A.ws->stats[5] = has_axis ? ring_radius_raw(A, mid) : 0.0;
-    A.ws->stats[6] = has_axis ? ring_radius(A, mid) : 0.0;
+    A.ws->stats[5] = axis_raw;
+    A.ws->stats[6] = axis_used;
     A.ws->stats[7] = lost;
   }
 }
