@@ -13,7 +13,8 @@
  *                   the Python binding); the library never allocates, frees or keeps it.  Pointers
  *                   named *_host are HOST memory owned by the caller.  Exceptions, stated where they occur:
  *                   gray_integrate_host keeps two streams and 80 bytes of pinned staging per device; the two
- *                   microbenchmarks gray_fma_peak / gray_packed_peak allocate and free a few KB while they run.
+ *                   microbenchmarks gray_fma_peak / gray_packed_peak allocate and free a few KB while they run;
+ *                   gray_shadow_edge_noalloc takes no workspace and uses a 128.5 KB array built into the library.
  *   layout          structure of arrays of 16-byte-aligned 4-vectors: x[p] = (t, r, theta, phi),
  *                   k[p] = (k^t, k^r, k^theta, k^phi); float4 for GRAY_F32, 4 doubles for GRAY_F64.
  *   stream          `cuda_stream` is a cudaStream_t passed as void* (NULL = the default stream).  All
@@ -235,6 +236,46 @@ typedef struct {
 GRAY_API int gray_shadow_edge(const gray_state* state, int32_t n_angles, double* radius_dev,
                      gray_shadow_stats* stats_host, void* workspace_dev, size_t workspace_bytes,
                      void* cuda_stream);
+
+/* gray_shadow_edge for callers that cannot allocate device memory, and so have no workspace_dev to pass.
+ *
+ * Who that is: code that runs on a GPU whose memory it does not manage.  A plug-in inside a host program (a
+ * visualisation tool, a simulation that calls libgray in situ) is typically handed its device buffers and forbidden
+ * cudaMalloc, because the host program gave the whole device to its own pool; a worker inside a fixed memory slice
+ * (MIG, an MPS limit, a scheduler's quota) that the photon buffers already fill has nothing left to ask for; and a
+ * frame loop like the paper's interactive mode cannot afford cudaMalloc / cudaFree, which stall every stream of
+ * the device while they run.  Every other entry point of this header expects such a caller to have set a workspace
+ * aside in advance; this one needs none.
+ *
+ * What it computes: exactly gray_shadow_edge (same statistics, same radius_dev[k], eqs. 6-8), from the
+ * same inputs (state: a full grid batch) into the same outputs (radius_dev, optional; stats_host).  The scratch memory
+ * the computation needs - the reduction cells and one radius per spoke - is an array built into libgray's device
+ * image: 512 B + 8 B x GRAY_NOALLOC_MAX_ANGLES = 128.5 KB, which every GPU that loads the library holds from then
+ * until the process exits, used or not.  That is why the limit is modest: n_angles > GRAY_NOALLOC_MAX_ANGLES
+ * (also returned by gray_noalloc_max_angles()) is refused with GRAY_ERR_ARG and a message that says so, before
+ * anything is launched; gray_shadow_edge with a workspace has no such limit.
+ *
+ * The call performs no cudaMalloc, cudaFree, cudaHostAlloc, stream / event creation or any other allocating
+ * runtime or library routine: argument checks, two cudaMemsetAsync, two kernels, two 64-byte copies into
+ * *stats_host, one cudaStreamSynchronize.
+ *
+ * First call on a device: the library asks the runtime where that device's copy of the array lives
+ * (cudaGetSymbolAddress, checked; each GPU has its own copy, so this is done once per device, with the device the
+ * caller has made current) and remembers the answer.  That look-up is a set-up step, not stream work: make the first
+ * call on each device early - before any stream capture is begun on it - and from then on the call only enqueues.
+ *
+ * One array per GPU, shared by every call: it still holds what the previous call left.  The cells that must start
+ * from zero (the sums, the captured count, the extreme columns) are cleared on `cuda_stream` at the start of each
+ * call and every spoke's radius is written before it is read, so consecutive calls on one stream, or calls
+ * separated by a synchronisation, are independent of each other.  Two calls of one process that can run on the
+ * same GPU at the same time (different streams, different host threads) write the same cells and RACE: serialise
+ * them yourself.  Another process has loaded its own copy of the array and does not interfere.
+ * Synchronises the stream.  Errors: GRAY_ERR_ARG (as gray_shadow_edge, or n_angles over the limit),
+ * GRAY_ERR_UNSUPPORTED (device ordinal >= 64), GRAY_ERR_CUDA.                                           */
+#define GRAY_NOALLOC_MAX_ANGLES 16384
+GRAY_API int gray_noalloc_max_angles(void);
+GRAY_API int gray_shadow_edge_noalloc(const gray_state* state, int32_t n_angles, double* radius_dev,
+                             gray_shadow_stats* stats_host, void* cuda_stream);
 
 /* Photon-ring statistics of a polar image (eqs. 6-10).  radius[k] = ring radius on spoke k: the outer
  * edge of the outermost captured cell (R_lo if none is captured).  alpha_max = radius[0], alpha_min = -radius[n_theta - 1]; D = |alpha_min + alpha_max| / 2

@@ -2,6 +2,8 @@
 // the shadow / photon-ring statistics of paper eqs. (6)-(8), from the per-photon status.
 #include "gray_internal.h"
 
+#include <mutex>
+
 namespace gray {
 
 __device__ __forceinline__ unsigned int warp_sum_u32(unsigned int v) { return __reduce_add_sync(0xffffffffu, v); }
@@ -271,6 +273,93 @@ static unsigned int reduce_grid(unsigned long long n, unsigned long long per_thr
   return (unsigned int)(blocks ? blocks : 1);
 }
 
+// ------------------------------------------------------------------ gray_shadow_edge_noalloc (gray.h)
+// The scratch memory of gray_shadow_edge, for callers that cannot hand the library a device workspace because they have
+// no way to allocate one: the reduction cells of the Workspace and one radius per spoke live in a file-scope device
+// array.  The driver reserves it on every GPU that loads libgray, from the moment the module is loaded until the
+// process ends, so it is kept small: 512 B + 8 B x GRAY_NOALLOC_MAX_ANGLES = 128.5 KB.
+struct NoAllocScratch {
+  Workspace ws;                              // sum_col .. n_captured and stats[] are used, as in gray_shadow_edge
+  double rho[GRAY_NOALLOC_MAX_ANGLES];       // rho(vartheta_k) between the two passes of the statistics kernel
+};
+static __device__ __align__(256) unsigned long long noalloc_scratch[(sizeof(NoAllocScratch) + 7) / 8];
+
+// shadow_edge_kernel with the radii of ALL spokes kept in the scratch array between the mean (eq. 7) and the variance
+// (eq. 8) pass, instead of the first 5120 in shared memory and the rest marched a second time.  Same arithmetic in the
+// same order, so the results are those of shadow_edge_kernel.  Every rho[k], k < n_angles, is written in the first pass
+// before the second reads it (by the same lane), so what an earlier call left there is never seen.
+__global__ void __launch_bounds__(1024) shadow_edge_scratch_kernel(const __grid_constant__ EdgeArgs A, double* __restrict__ rho_scratch) {
+  __shared__ double sh[32];
+  Workspace* ws = A.ws;
+  const double da = 2.0 * A.W / (double)A.nx, db = 2.0 * A.W / (double)A.ny;
+  const double delta = fmin(da, db) / 2.0;
+  const unsigned long long ncap = ws->n_captured;
+  const double amin = ncap ? -A.W + (double)ws->min_col * da : 0.0;
+  const double amax = ncap ? -A.W + (double)(ws->max_col + 1) * da : 0.0;
+  const double centre = (amin + amax) / 2.0;
+  const double two_pi = 2.0 * 3.14159265358979323846;
+  const int warp = threadIdx.x >> 5, n_warps = blockDim.x >> 5, lane = threadIdx.x & 31;
+  auto R_of = [&](int k, double rho) {
+    const double vt = two_pi * ((double)k + 0.5) / (double)A.n_angles;
+    double sv, cv;
+    sincos(vt, &sv, &cv);
+    const double x = rho * cv - centre, y = rho * sv;
+    return sqrt(x * x + y * y);
+  };
+  double sumR = 0.0;
+  for (int k = warp; k < A.n_angles; k += n_warps) {
+    const double vt = two_pi * ((double)k + 0.5) / (double)A.n_angles;
+    double sv, cv;
+    sincos(vt, &sv, &cv);
+    const double rho = spoke_radius_warp(A, da, db, delta, cv, sv);
+    if (lane == 0) {
+      rho_scratch[k] = rho;
+      if (A.radius) A.radius[k] = rho;
+      sumR += R_of(k, rho);
+    }
+  }
+  const double mean = A.n_angles > 0 ? block_sum(sumR, sh) / (double)A.n_angles : 0.0;     // (block_sum synchronises)
+  double var = 0.0;
+  for (int k = warp; k < A.n_angles; k += n_warps) {
+    if (lane == 0) {
+      const double d = R_of(k, rho_scratch[k]) - mean;
+      var += d * d;
+    }
+  }
+  var = A.n_angles > 0 ? block_sum(var, sh) / (double)A.n_angles : 0.0;
+  if (threadIdx.x == 0) {
+    ws->stats[0] = (double)ncap * da * db;
+    ws->stats[1] = ncap ? -A.W + ((double)ws->sum_col / (double)ncap + 0.5) * da : 0.0;
+    ws->stats[2] = ncap ? -A.W + ((double)ws->sum_row / (double)ncap + 0.5) * db : 0.0;
+    ws->stats[3] = amin;
+    ws->stats[4] = amax;
+    ws->stats[5] = fabs(amin + amax) / 2.0;
+    ws->stats[6] = mean;
+    ws->stats[7] = 2.0 * sqrt(var);
+  }
+}
+
+// Device address of noalloc_scratch on the current device.  In host code the name `noalloc_scratch` is only the
+// runtime's handle for the symbol, not memory a kernel could use: the address has to be asked for, once per device
+// (each GPU has its own copy of the array), with that device current.
+constexpr int kNoAllocMaxDevices = 64;
+static std::mutex g_noalloc_mutex;
+static NoAllocScratch* g_noalloc_ptr[kNoAllocMaxDevices];
+static int noalloc_scratch_on_current_device(NoAllocScratch** out) {
+  int dev = -1;
+  GRAY_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kNoAllocMaxDevices) { set_error("gray_shadow_edge_noalloc: device ordinal %d is not below %d", dev, kNoAllocMaxDevices); return GRAY_ERR_UNSUPPORTED; }
+  std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+  if (!g_noalloc_ptr[dev]) {
+    void* p = nullptr;
+    GRAY_CUDA(cudaGetSymbolAddress(&p, noalloc_scratch));
+    if (!p || ((uintptr_t)p & 255)) { set_error("gray_shadow_edge_noalloc: the runtime gave no usable address for the static scratch array"); return GRAY_ERR_CUDA; }
+    g_noalloc_ptr[dev] = (NoAllocScratch*)p;
+  }
+  *out = g_noalloc_ptr[dev];
+  return GRAY_OK;
+}
+
 }  // namespace gray
 
 extern "C" {
@@ -361,6 +450,55 @@ int gray_ring_polar(const gray_state* state, int32_t bridge_axis, double* radius
   stats_host->alpha_min = s[0]; stats_host->alpha_max = s[1]; stats_host->D = s[2];
   stats_host->R_mean = s[3]; stats_host->A = s[4];
   stats_host->axis_radius_traced = s[5]; stats_host->axis_radius_used = s[6]; stats_host->axis_rays_lost = (uint64_t)s[7];
+  return GRAY_OK;
+}
+
+int gray_noalloc_max_angles(void) { return GRAY_NOALLOC_MAX_ANGLES; }
+
+// gray_shadow_edge without a caller-supplied workspace (gray.h).  Nothing in here allocates or frees: argument checks,
+// one address look-up the first time a device is seen, two memsets, two kernels, two small copies to the caller's host
+// struct, one stream synchronisation.
+int gray_shadow_edge_noalloc(const gray_state* state, int32_t n_angles, double* radius_dev, gray_shadow_stats* stats_host,
+                             void* cuda_stream) {
+  using namespace gray;
+  int rc = check_state(state, true);
+  if (rc) return rc;
+  if (!stats_host || n_angles < 0) { set_error("stats_host is NULL or n_angles < 0"); return GRAY_ERR_ARG; }
+  if (n_angles > GRAY_NOALLOC_MAX_ANGLES) {
+    set_error("gray_shadow_edge_noalloc: n_angles = %d is more than the %d spokes the static scratch array holds "
+              "(GRAY_NOALLOC_MAX_ANGLES); use gray_shadow_edge with a workspace of your own for more", (int)n_angles,
+              (int)GRAY_NOALLOC_MAX_ANGLES);
+    return GRAY_ERR_ARG;
+  }
+  if (state->pixels != GRAY_PIXELS_GRID || state->p0 != 0 || state->nx <= 0 || state->ny <= 0 ||
+      state->n != (uint64_t)state->nx * (uint64_t)state->ny) {
+    set_error("gray_shadow_edge_noalloc needs a full grid image (pixels = GRID, p0 = 0, n = nx * ny)");
+    return GRAY_ERR_ARG;
+  }
+  NoAllocScratch* scratch = nullptr;
+  rc = noalloc_scratch_on_current_device(&scratch);
+  if (rc) return rc;
+  cudaStream_t stream = (cudaStream_t)cuda_stream;
+  Workspace* ws = &scratch->ws;
+  // the array still holds the previous call's sums: the cells the reduction adds into start at zero, min_col at the maximum
+  GRAY_CUDA(cudaMemsetAsync(&ws->sum_col, 0, (char*)&ws->pad3[0] - (char*)&ws->sum_col, stream));
+  GRAY_CUDA(cudaMemsetAsync(&ws->min_col, 0xff, sizeof ws->min_col, stream));
+  shadow_reduce_kernel<<<reduce_grid(state->n, 4), 256, 0, stream>>>(state->status_dev, state->n, (unsigned int)state->nx, ws);
+  GRAY_CUDA(cudaGetLastError());
+  EdgeArgs A;
+  A.status = state->status_dev; A.nx = state->nx; A.ny = state->ny; A.W = state->half_width;
+  A.n_angles = n_angles; A.radius = radius_dev; A.ws = ws;
+  shadow_edge_scratch_kernel<<<1, 1024, 0, stream>>>(A, scratch->rho);
+  GRAY_CUDA(cudaGetLastError());
+  double s[8];
+  unsigned long long ncap = 0;
+  GRAY_CUDA(cudaMemcpyAsync(s, &ws->stats[0], sizeof s, cudaMemcpyDeviceToHost, stream));
+  GRAY_CUDA(cudaMemcpyAsync(&ncap, &ws->n_captured, sizeof ncap, cudaMemcpyDeviceToHost, stream));
+  GRAY_CUDA(cudaStreamSynchronize(stream));
+  stats_host->area = s[0]; stats_host->centroid_alpha = s[1]; stats_host->centroid_beta = s[2];
+  stats_host->alpha_min = s[3]; stats_host->alpha_max = s[4]; stats_host->D = s[5];
+  stats_host->R_mean = s[6]; stats_host->A = s[7];
+  stats_host->n_captured = ncap;
   return GRAY_OK;
 }
 

@@ -77,6 +77,10 @@ def lib():
         L.gray_integrate_counters.argtypes = [vp, C.POINTER(_Counters), vp]
         L.gray_classify.argtypes = [C.POINTER(_State), vp, C.POINTER(u64), vp, C.c_size_t, vp]
         L.gray_shadow_edge.argtypes = [C.POINTER(_State), i32, vp, C.POINTER(_ShadowStats), vp, C.c_size_t, vp]
+        L.gray_shadow_edge_noalloc.argtypes = [C.POINTER(_State), i32, vp, C.POINTER(_ShadowStats), vp]
+        L.gray_shadow_edge_noalloc.restype = C.c_int
+        L.gray_noalloc_max_angles.argtypes = []
+        L.gray_noalloc_max_angles.restype = C.c_int
         L.gray_host_scratch_bytes.argtypes = [u64, i32]
         L.gray_host_scratch_bytes.restype = C.c_size_t
         L.gray_integrate_host.argtypes = [vp, vp, vp, vp, vp, vp, u64, i32, dbl, dbl, C.c_uint32, C.POINTER(_StepParams),
@@ -218,6 +222,22 @@ def gray_shadow_edge(batch, n_angles, radius=None):
     s = _ShadowStats()
     _check(lib().gray_shadow_edge(C.byref(batch.c), n_angles, _ptr(radius), C.byref(s), _ptr(batch.workspace),
                                   batch.workspace.numel(), _stream()))
+    return {k: getattr(s, k) for k, _ in _ShadowStats._fields_}
+
+
+def gray_noalloc_max_angles():
+    """Most spokes gray_shadow_edge_noalloc accepts (GRAY_NOALLOC_MAX_ANGLES of include/gray.h)."""
+    return int(lib().gray_noalloc_max_angles())
+
+
+def gray_shadow_edge_noalloc(batch, n_angles, radius=None):
+    """gray_shadow_edge for a caller that may not allocate device memory (a plug-in whose host program owns the
+    GPU's memory pool, a worker whose memory slice is already full, a frame loop that cannot stall on cudaMalloc):
+    batch.workspace is NOT used, the scratch memory is an array built into libgray.so (include/gray.h has the details:
+    at most gray_noalloc_max_angles() spokes, one call at a time per GPU, first call on a device does a one-off address
+    look-up).  Same results as gray_shadow_edge: the stats as a dict; fills radius (float64 tensor of n_angles) if given."""
+    s = _ShadowStats()
+    _check(lib().gray_shadow_edge_noalloc(C.byref(batch.c), n_angles, _ptr(radius), C.byref(s), _stream()))
     return {k: getattr(s, k) for k, _ in _ShadowStats._fields_}
 
 
