@@ -189,9 +189,13 @@ GRAY_API size_t gray_workspace_bytes(uint64_t n);
  * is carried in variables that the stored (t, r, theta, phi; k) do not hold exactly: the height above the horizon
  * d = r - r_bh, the polar angle folded into [0, pi/2], and (GRAY_F32) the compensation terms of the state update.
  *   state->resume_dev != NULL  these are saved for every photon left LIVE (64 B per photon in fp32, 128 B in fp64)
- *                              and restored by the next call if the record still matches the stored r, theta and
- *                              step count bit for bit (so a state edited by the caller is simply re-read): any
- *                              sequence of calls then gives results BIT-IDENTICAL to one uninterrupted call.
+ *                              and restored by the next call if the record still matches the stored r, theta, k^mu
+ *                              and step count bit for bit and was written for the same `system`: any sequence of
+ *                              calls with the same parameters then gives results BIT-IDENTICAL to one uninterrupted
+ *                              call.  A photon whose stored r, theta, any k^mu or step count the caller has edited,
+ *                              or that the previous call advanced with the other gray_system, is re-read from
+ *                              (x, k) like a fresh one (an edit of t or phi alone keeps the record: they feed nothing
+ *                              back, and the edited value is the one integrated on).
  *   state->resume_dev == NULL  each interruption rounds r and theta once and drops the compensation: results agree
  *                              with the uninterrupted call to rounding error amplified along the ray (within the
  *                              tolerances of the build, tests/test_gpu_parity.py), not bit for bit.

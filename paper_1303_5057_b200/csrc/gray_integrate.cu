@@ -23,6 +23,25 @@ __device__ __forceinline__ double bits_to_scalar(unsigned long long b, double) {
 __device__ __forceinline__ unsigned long long scalar_bits(float v) { return __float_as_uint(v); }
 __device__ __forceinline__ unsigned long long scalar_bits(double v) { return (unsigned long long)__double_as_longlong(v); }
 constexpr unsigned long long kResumeMagic = 0x47524159ull;       // "GRAY"
+// Key word of a resume record: the magic mixed with the bits of the four stored k^mu and with the system (full / reduced)
+// that wrote the record, in the width of the scalar.  A record is only taken back by a call that finds the very k it was
+// written next to and integrates the same system: a caller who edits k (say, reverses a ray), or who switches
+// GRAY_SYS_FULL <-> GRAY_SYS_REDUCED between calls, gets the photon rebuilt from (x, k) instead of stale compensation
+// terms or stale constants E, L.
+__device__ __forceinline__ unsigned long long resume_key(float kt, float kr, float kh, float kp, bool red) {
+  unsigned int h = (unsigned int)kResumeMagic ^ (red ? 0x52454455u : 0u);      // "REDU"
+  const unsigned int w[4] = {__float_as_uint(kt), __float_as_uint(kr), __float_as_uint(kh), __float_as_uint(kp)};
+#pragma unroll
+  for (int i = 0; i < 4; ++i) { h = (h ^ w[i]) * 0x9e3779b1u; h ^= h >> 15; }
+  return h;
+}
+__device__ __forceinline__ unsigned long long resume_key(double kt, double kr, double kh, double kp, bool red) {
+  unsigned long long h = kResumeMagic ^ (red ? 0x5245445500000000ull : 0ull);
+  const unsigned long long w[4] = {scalar_bits(kt), scalar_bits(kr), scalar_bits(kh), scalar_bits(kp)};
+#pragma unroll
+  for (int i = 0; i < 4; ++i) { h = (h ^ w[i]) * 0xff51afd7ed558ccdull; h ^= h >> 33; }
+  return h;
+}
 
 template <typename V>
 struct IntegrateArgs {
@@ -135,14 +154,15 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
 #pragma unroll
       for (int i = 0; i < 8; ++i) cs[i][l] = S(0);
       // A photon left LIVE by an earlier call that wrote a resume record (gray.h): if the record belongs to exactly
-      // this stored state (same r, theta bits, same step count), the kernel's own variables - d, the folded theta,
-      // the compensation terms, E and L of the reduced system - are taken from it, and the continuation is
-      // bit-identical to an uninterrupted run.  Otherwise they are rebuilt from (r, theta) as above.
+      // this stored state (same r, theta bits, same step count, same k and same system through resume_key), the
+      // kernel's own variables - d, the folded theta, the compensation terms, E and L of the reduced system - are
+      // taken from it, and the continuation is bit-identical to an uninterrupted run.  Otherwise they are rebuilt
+      // from (x, k) as above.
       bool resumed = false;
       if (A.resume != nullptr) {
         const typename Vec4T<S>::type r3 = A.resume[4 * p + 3];
         if (scalar_bits(r3.x) == scalar_bits(xv.y) && scalar_bits(r3.y) == scalar_bits(xv.z) &&
-            scalar_bits(r3.z) == (unsigned long long)s && scalar_bits(r3.w) == kResumeMagic) {
+            scalar_bits(r3.z) == (unsigned long long)s && scalar_bits(r3.w) == resume_key(kv.x, kv.y, kv.z, kv.w, RED)) {
           const typename Vec4T<S>::type r0 = A.resume[4 * p], r1 = A.resume[4 * p + 1], r2 = A.resume[4 * p + 2];
           const unsigned long long flags = scalar_bits(r2.w);
           m = (int)(flags & 1ull);
@@ -194,7 +214,7 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
       r1.x = vget(comp[1], l); r1.y = vget(comp[2], l); r1.z = vget(comp[3], l); r1.w = RED ? S(0) : vget(comp[4], l);
       r2.x = vget(comp[5], l); r2.y = vget(comp[6], l); r2.z = RED ? S(0) : vget(comp[7], l);
       r2.w = bits_to_scalar(mirrored[l] ? 1ull : 0ull, S(0));
-      r3.x = xv.y; r3.y = xv.z; r3.z = bits_to_scalar((unsigned long long)nst[l], S(0)); r3.w = bits_to_scalar(kResumeMagic, S(0));
+      r3.x = xv.y; r3.y = xv.z; r3.z = bits_to_scalar((unsigned long long)nst[l], S(0)); r3.w = bits_to_scalar(resume_key(kv.x, kv.y, kv.z, kv.w, RED), S(0));
       A.resume[4 * p] = r0; A.resume[4 * p + 1] = r1; A.resume[4 * p + 2] = r2; A.resume[4 * p + 3] = r3;
     }
     c_steps += nst[l] - nst0[l];

@@ -7,6 +7,7 @@ import closed_forms as cf
 import oracle as o
 import paper_1303_5057_b200 as g
 from gpu_common import edge_band, exact_capture, gpu_state, grid_pixels, pole_band, rel_err_final, upload_state, xi_eta_of
+import xi_cases
 from paper_1303_5057_b200 import workloads as wl
 
 pytestmark = pytest.mark.gpu
@@ -330,6 +331,53 @@ def test_resumed_calls_are_bit_identical_with_resume_records(prec, kw):
 
 
 @pytest.mark.parametrize("prec", [g.GRAY_F32, g.GRAY_F64])
+def test_resume_record_is_keyed_by_system_and_by_the_stored_k(prec):
+    # ADVICE r2 (gray_integrate.cu take()): a record belongs to the system that wrote it and to the k^mu stored next to
+    # it.  A call with the other gray_system, or after the caller has edited nothing but k, must rebuild the photon
+    # from (x, k) - i.e. behave exactly like a batch that carries the same stored state and no records at all -
+    # instead of taking E = L = 0 (full -> reduced), stale E, L (reduced, k edited) or stale compensation terms.
+    a, inc, W, nx, ny = 0.9, 60.0, 10.0, 90, 31
+    n = nx * ny
+
+    def interrupted(system):
+        b = g.PhotonBatch(n, prec, resumable=True)
+        g.gray_init_rays(b, a, wl.R_OBS, inc, W, nx, ny)
+        g.gray_integrate(b, max_steps=100, params=g.StepParams(rule=g.STEP_EQ2, system=system))
+        c = g.PhotonBatch(n, prec)                                # the same stored state, no records
+        for dst, src in ((c.x, b.x), (c.k, b.k), (c.status, b.status), (c.steps, b.steps)):
+            dst.copy_(src)
+        c.set_image_plane(a, wl.R_OBS, inc, W, nx, ny)
+        return b, c
+
+    def finish_and_compare(b, c, system, what):
+        for q in (b, c):
+            g.gray_integrate(q, max_steps=wl.MAX_STEPS, params=g.StepParams(rule=g.STEP_EQ2, system=system))
+        assert g.gray_classify(b)[g.LIVE] == 0
+        for u, v in ((b.x, c.x), (b.k, c.k), (b.status, c.status), (b.steps, c.steps)):
+            assert torch.equal(u.view(torch.uint8), v.view(torch.uint8)), what
+
+    for first, second in ((g.SYS_FULL, g.SYS_REDUCED), (g.SYS_REDUCED, g.SYS_FULL)):
+        b, c = interrupted(first)
+        finish_and_compare(b, c, second, ("system", first, second))
+    for system in (g.SYS_FULL, g.SYS_REDUCED):
+        b, c = interrupted(system)
+        for q in (b, c):
+            q.k[:, 3] *= 1.0 + 2.0 ** -10                         # the caller edits k^phi and nothing else
+        finish_and_compare(b, c, system, ("k^phi edited", system))
+        b, c = interrupted(system)
+        for q in (b, c):
+            q.k[:, 1] *= 1.0 - 2.0 ** -10                         # ... or k^r
+        finish_and_compare(b, c, system, ("k^r edited", system))
+    # and an untouched record is still taken: the edit-free continuation differs from the record-free one in fp32
+    # (compensation terms dropped) while both finish every ray
+    b, c = interrupted(g.SYS_FULL)
+    for q in (b, c):
+        g.gray_integrate(q, max_steps=wl.MAX_STEPS, params=g.StepParams(rule=g.STEP_EQ2))
+    if prec == g.GRAY_F32:
+        assert not torch.equal(b.x.view(torch.uint8), c.x.view(torch.uint8))
+
+
+@pytest.mark.parametrize("prec", [g.GRAY_F32, g.GRAY_F64])
 def test_resumed_calls_without_records_stay_within_the_parity_tolerances(prec):
     # Without resume_dev every interruption rounds r = d + r_h and theta once and (fp32) drops the compensation terms
     # (gray.h; reading R22).  Bound, not bit-identity: after sixty interruptions (fifty 20-step calls, then
@@ -469,6 +517,44 @@ def test_xi_monitor_one_step_branches_match_oracle(prec, ppt):
     y, _, _ = gpu_state(b)
     err = np.max(np.abs(y - want_rk) / np.maximum(np.abs(want_rk), 1.0), axis=1)
     assert err.max() <= (2e-6 if f32 else 1e-12), err.max()
+
+
+@pytest.mark.parametrize("prec", [g.GRAY_F32, g.GRAY_F64])
+def test_paper_pole_test_ray_of_fig2(prec):
+    # P:91-107, Fig. 2; SURVEY 8(f) NEXT-1 "regression on the P:91 test ray".  The oracle side of this regression is
+    # test_oracle_integrate.py::test_paper_pole_test_ray_of_fig2 (what it reproduces of the figure, and why every one of
+    # these rays should be captured).  Here: the kernel against the oracle on the same four rays.
+    a, r_obs = xi_cases.GOLD["pole_ray_spin"], xi_cases.GOLD["pole_ray_height"]
+    f32 = prec == g.GRAY_F32
+    y0 = np.array([o.init_ray(a, r_obs, 0.0, al, be) for al, be in xi_cases.paper_pole_rays()])
+    if f32:
+        y0 = y0.astype(np.float32).astype(np.float64)
+    got, want = {}, {}
+    for eps in (0.0, xi_cases.EPS):
+        b = g.PhotonBatch(len(y0), prec)
+        upload_state(b, y0)
+        b.set_image_plane(a, r_obs, 0.0, 10.0)
+        g.gray_integrate(b, max_steps=wl.MAX_STEPS, params=g.StepParams(rule=g.STEP_EQ2, xi_epsilon=eps))
+        _, st, ns = gpu_state(b)
+        ref = [o.integrate(a, v, xi_cases.H, 1.01 * o.horizon(a), 1.01 * r_obs, o.STEP_EQ2, wl.MAX_STEPS, xi_eps=eps)[1:] for v in y0]
+        got[eps], want[eps] = (st, ns), (np.array([r[0] for r in ref]), np.array([r[1] for r in ref]))
+    # with the paper's monitor: every ray captured, on both sides (the red trajectory)
+    assert np.all(got[xi_cases.EPS][0] == g.CAPTURED) and np.all(want[xi_cases.EPS][0] == o.CAPTURED)
+    # the printed ray and its azimuthal copy: the same status as the oracle with and without the monitor
+    for eps in got:
+        assert np.array_equal(got[eps][0][:2], want[eps][0][:2])
+        assert got[eps][1][0] == got[eps][1][1]                       # phi0 does not matter
+    # (3.0, -3.79) without the monitor: kicked back to infinity on both sides (the blue trajectory)
+    assert got[0.0][0][2] == g.ESCAPED == want[0.0][0][2]
+    if not f32:
+        # fp64: the kernel follows the oracle's trajectory through both poles and the windings, status for status;
+        # step counts to within 1 % (these rays wind on the unstable photon orbit, which amplifies the 1e-12 differences
+        # of a step: the printed ray takes the oracle's 1199 / 2550 steps exactly, (3.0, -3.79) 2120 for 2119, the ray
+        # at 4.82 M - whose Euler fallback steps the winding amplifies most - 1322 for 1332)
+        for eps in got:
+            assert np.array_equal(got[eps][0], want[eps][0])
+            assert np.all(np.abs(got[eps][1] - want[eps][1]) <= 0.01 * want[eps][1]), (got[eps][1], want[eps][1])
+        assert np.array_equal(got[0.0][1][:2], want[0.0][1][:2]) and np.array_equal(got[xi_cases.EPS][1][:2], want[xi_cases.EPS][1][:2])
 
 
 # ------------------------------------------------------------------------ classify / shadow

@@ -5,6 +5,7 @@ import pytest
 import closed_forms as cf
 import golden_values
 import oracle as o
+import xi_cases
 
 GOLD = golden_values.load()
 
@@ -242,6 +243,41 @@ def test_pole_treatment_xi_monitor_cures_the_pole_failures():
     c2 = o.trace(a, 1000.0, inc, W, nx, nx, idx=idx2, rule=o.STEP_EQ2, xi_eps=1e-3)
     esc = p2["status"] == o.ESCAPED
     assert esc.any() and np.array_equal(p2["y"][esc], c2["y"][esc]) and np.array_equal(p2["steps"][esc], c2["steps"][esc])
+
+
+def test_paper_pole_test_ray_of_fig2():
+    # P:91-107, Fig. 2 ("regression on the P:91 test ray").  The printed ray starts at
+    # r0 cos(theta0) = 1000 M, r0 sin(theta0) = 4.833605 M, phi0 = 0 above a spin 0.99 hole and "passes both the south
+    # and north poles"; the red (monitored) trajectory "eventually hit[s] the event horizon", the blue (plain RK4) one
+    # "is kicked back to infinity".  What the oracle must and does reproduce:
+    a, r_obs = GOLD["pole_ray_spin"], GOLD["pole_ray_height"]
+    rays = xi_cases.paper_pole_rays()
+    y0 = np.array([o.init_ray(a, r_obs, 0.0, al, be) for al, be in rays])
+    assert abs(y0[0, 1] * np.cos(y0[0, 2]) - r_obs) < 1e-9 and abs(y0[0, 1] * np.sin(y0[0, 2]) - GOLD["pole_ray_impact"]) < 1e-10
+    assert y0[0, 3] == 0.0 and abs(y0[1, 3] - np.pi / 2) < 1e-15
+    inv = np.array([o.invariants(a, v) for v in y0])
+    assert np.max(np.abs(inv[:, 1])) < 1e-7                                   # L_z = g_t_phi k^t ~ -5e-8: rays through the axis
+    assert all(cf.captured_exact(a, L / E, Q / E ** 2) for E, L, Q, _ in inv)   # the exact answer: captured
+    run = lambda y, eps: o.integrate(a, y, GOLD["step_parameter"], 1.01 * o.horizon(a), 1.01 * r_obs, o.STEP_EQ2, 20000,
+                                     xi_eps=eps)
+    # (i) the south pole is passed first, then the north pole: theta leaves [0, pi] above, later below (plain steps
+    # written out with the pinned pieces; the remap of eq. (3) folds it back)
+    y, crossings = y0[0].copy(), []
+    for _ in range(1100):
+        y = o.rk4_step(a, y, o.step_size(a, y, GOLD["step_parameter"], o.STEP_EQ2))
+        if y[2] > np.pi or y[2] < 0.0:
+            crossings.append("S" if y[2] > np.pi else "N")
+        y = o.remap_theta(y)
+    assert crossings[:2] == ["S", "N"], crossings
+    # (ii) with the monitor (epsilon = 1e-3) every one of the rays is captured, after a couple of windings
+    mon = [run(v, GOLD["xi_epsilon"]) for v in y0]
+    assert all(st == o.CAPTURED for _, st, _ in mon)
+    assert mon[0][2] == mon[1][2] and mon[0][2] > 2000                        # phi0 does not matter; > 2 windings' worth of steps
+    # (iii) without it, the blue trajectory: neighbours 3e-5 and 3e-3 M away are kicked back to infinity, although
+    # they too lie inside the critical radius (the printed ray itself survives the poles in this implementation)
+    plain = [run(v, 0.0) for v in y0]
+    assert [st for _, st, _ in plain] == [o.CAPTURED, o.CAPTURED, o.ESCAPED, o.ESCAPED]
+    assert abs(plain[2][0][1] - 1.01 * r_obs) < 0.1 * r_obs                   # ... all the way out
 
 
 def test_xi_monitor_fallback_is_one_euler_step_of_a_ninth_from_the_old_state():
