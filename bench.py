@@ -116,8 +116,9 @@ class ClockSampler:
 def workload_config(args, world):
     from paper_1303_5057_b200 import workloads as wl
     c4 = wl.C4
-    return {"workload": f"C4-{args.case}: 2^{args.log2n} photons/GPU, Kerr a={c4['a']}, i={c4['inc_deg']} deg, seeded random "
-                        f"pixels over +-{c4['half_width']} M at r_obs={wl.R_OBS:.0f} M, RK4 h=1/32, rule={args.rule}",
+    # (rule first, under 120 characters: the driver's record keeps that much of the string)
+    return {"workload": f"C4-{args.case} rule={args.rule}: 2^{args.log2n} photons/GPU, Kerr a={c4['a']} i={c4['inc_deg']:g} deg, "
+                        f"random pixels +-{c4['half_width']:g} M, r_obs={wl.R_OBS:.0f} M, RK4 h=1/32",
             "photons_per_gpu": 2 ** args.log2n, "photons_total": world * 2 ** args.log2n, "precision": args.prec,
             "step_rule": args.rule, "case": args.case, "schedule": args.schedule, "xi_epsilon": args.xi_eps, "system": args.system, "max_steps": wl.MAX_STEPS if args.case == "realistic" else c4["peak_steps"],
             "seed": c4["seed"], "parallelism": f"photon-range sharding x{world}, no collective on the data path",
@@ -161,7 +162,8 @@ def run_reference(args):
     out = {"impl": "reference", "metric": "photon-steps/s", "value": value, "unit": "photon-steps/s", "n_gpus": args.gpus,
            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps, "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-           "config": dict(workload_config(args, 1), precision="f64 (the oracle's arithmetic; the GPU arm's is f32)"),
+           "config": workload_config(args, 1),
+           "note": "the oracle computes in f64 (dtype) whatever config.precision says: that key names the GPU arm's build",
            "ns_per_photon_step": 1e9 / value,
            "cpu_baseline": {"value": value, "unit": "photon-steps/s", "cores": threads, "kind": "oracle", "sample": sample},
            "e2e": {"value": value, "unit": "photon-steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
