@@ -287,4 +287,23 @@ void gray_oracle_op_tally(double a, const double* y, double h, int rule, uint64_
   counts7[4] = t.sin_; counts7[5] = t.cos_; counts7[6] = t.other;
 }
 
+// The same tally for either system (0 = full as above, 1 = reduced: step size + rk4_step_reduced, whose four stages and
+// final state each rebuild k^t, k^phi with killing_velocities, + remap).  E and L of the ray are formed once per ray
+// (integrate()), not per step, and are not counted.  Bookkeeping only: no arithmetic of the method changes.
+void gray_oracle_op_tally_system(double a, const double* y, double h, int rule, int system, uint64_t* counts7) {
+  using go::Counted;
+  if (system != go::SYS_REDUCED) { gray_oracle_op_tally(a, y, h, rule, counts7); return; }
+  double inv[4];
+  go::invariants(a, y, inv);
+  Counted yc[8];
+  for (int i = 0; i < 8; ++i) yc[i] = Counted(y[i]);
+  go::g_tally = go::Tally();
+  Counted dl = go::step_size(Counted(a), yc, Counted(h), rule);
+  go::rk4_step_reduced(Counted(a), Counted(inv[0]), Counted(inv[1]), yc, dl);
+  go::remap_theta(yc);
+  const go::Tally& t = go::g_tally;
+  counts7[0] = t.add; counts7[1] = t.mul; counts7[2] = t.div; counts7[3] = t.sqrt_;
+  counts7[4] = t.sin_; counts7[5] = t.cos_; counts7[6] = t.other;
+}
+
 }  // extern "C"

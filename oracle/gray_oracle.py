@@ -53,6 +53,7 @@ def lib():
         L.gray_oracle_ring_polar.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_double, C.c_double, C.c_int,
                                              C.c_void_p, C.c_void_p]
         L.gray_oracle_op_tally.argtypes = [C.c_double, _dp, C.c_double, C.c_int, C.POINTER(C.c_uint64)]
+        L.gray_oracle_op_tally_system.argtypes = [C.c_double, _dp, C.c_double, C.c_int, C.c_int, C.POINTER(C.c_uint64)]
         _lib = L
     return _lib
 
@@ -219,9 +220,9 @@ def pixel_polar(R_lo, R_hi, n_R, n_theta, p):
     return al.value, be.value
 
 
-def op_tally(a, y, h, rule):
+def op_tally(a, y, h, rule, system=SYS_FULL):
     """Operation counts of one photon-step: dict(add, mul, div, sqrt, sin, cos, other)."""
     y = _vec(y, 8)
     c = (C.c_uint64 * 7)()
-    lib().gray_oracle_op_tally(a, y.ctypes.data_as(_dp), h, rule, c)
+    lib().gray_oracle_op_tally_system(a, y.ctypes.data_as(_dp), h, rule, system, c)
     return dict(zip(["add", "mul", "div", "sqrt", "sin", "cos", "other"], [int(v) for v in c]))

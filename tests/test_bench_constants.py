@@ -16,6 +16,10 @@ def test_flops_per_photon_step_is_the_oracle_tally():
     for name, rule in (("rel", o.STEP_REL), ("eq2", o.STEP_EQ2)):
         t = o.op_tally(0.7, y, 1 / 32, rule)
         assert bench.FLOPS_PER_PHOTON_STEP[name] == t["add"] + t["mul"] + t["div"] + t["sqrt"] + t["sin"] + t["cos"]
+        t = o.op_tally(0.7, y, 1 / 32, rule, o.SYS_REDUCED)
+        assert bench.FLOPS_PER_PHOTON_STEP_REDUCED[name] == t["add"] + t["mul"] + t["div"] + t["sqrt"] + t["sin"] + t["cos"]
+        # the reduced oracle = the full one + five (k^t, k^phi) reconstructions: 4 stages + the final state
+        assert t["sin"] == 9 and t["cos"] == 9
     assert abs(bench.PEAK_TFLOPS["f32"] - 74.45) < 0.05 and abs(bench.PEAK_TFLOPS["f64"] - 37.2) < 0.05
 
 
