@@ -292,12 +292,16 @@ void init_ray(T a, T r_obs, T inc_rad, T alpha, T beta, T y[8]) {
   T yy = alpha;
   T z = r_obs * ci + beta * si;
   T r = sqrt(x * x + yy * yy + z * z);
-  T th = acos(z / r);
+  T q = sqrt(x * x + yy * yy);          // distance from the spin axis, r sin(theta)
+  T th = atan2(q, z);                   // (not acos(z / r): near the axis acos loses half the digits; reading R23)
   T ph = atan2(yy, x);
   T s = sin(th), c = cos(th);
   T kr = r_obs / r;
   T kh = (si * c * cos(ph) - ci * s) / r;
   T kp = -si * sin(ph) / (r * s);
+  // a pixel exactly on the spin axis (face-on observer, alpha = beta = 0) has no azimuth; the direction o is then
+  // parallel to the axis and its theta and phi components vanish in the limit (reading R23)
+  if (q == T(0)) { kh = T(0); kp = T(0); }
   T g[4][4];
   metric(a, r, th, g);
   // g_tt kt^2 + 2 g_tp kp kt + C = 0 with C the spatial part

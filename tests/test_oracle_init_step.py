@@ -48,6 +48,33 @@ def test_init_ray_null_E1_and_bardeen_impact_parameters(a, inc):
     assert worst[0] < 3e-2 and worst[1] < 0.35, worst
 
 
+def test_init_ray_for_observers_on_and_next_to_the_spin_axis():
+    # Reading R23.  For i = 0 and i = 0.1 deg the polar angle of a pixel is ~ rho / r_obs ~ 1e-3: theta from atan2 keeps
+    # r sin(theta) - the quantity every 1 / sin(theta) of the right-hand side divides by - to rounding (acos(z / r)
+    # would lose half the digits there); the state stays null with E = 1; and the central pixel of the face-on image
+    # (no azimuth: o is parallel to the axis) gets theta = 0, k^theta = k^phi = 0, all finite.
+    a = 0.9
+    for inc in (0.0, 0.1, 179.9, 180.0):
+        i = np.deg2rad(inc)
+        for al, be in ((3.0, 4.0), (-0.5, 0.002), (1e-3, -2e-3), (4.833605, 0.0)):
+            y = o.init_ray(a, 1000.0, inc, al, be)
+            X, Y, Z = 1000 * np.sin(i) - be * np.cos(i), al, 1000 * np.cos(i) + be * np.sin(i)
+            q = np.hypot(X, Y)
+            assert abs(y[1] * np.sin(y[2]) - q) <= 4e-16 * 1000.0          # a few ulp of r, i.e. 1e-13 relative at q = 5
+            assert abs(y[1] * np.cos(y[2]) - Z) <= 4e-13 and abs(y[3] - np.arctan2(Y, X)) <= 1e-15
+            E, L, Q, null = o.invariants(a, y)
+            assert abs(null) < 1e-14 and abs(E - 1) < 1e-13
+            # velocity parallel to the observer's axis, in Cartesian components (curvature corrections ~ 1/r_obs)
+            r, th, ph, kr, kh, kp = y[1], y[2], y[3], y[5], y[6], y[7]
+            vz = kr * np.cos(th) - r * kh * np.sin(th)
+            vq = kr * np.sin(th) + r * kh * np.cos(th)
+            assert abs(vz / np.hypot(vz, vq) - np.cos(i)) < 1e-2 and abs(r * kp * np.sin(th)) < 2e-3
+    for inc, th0 in ((0.0, 0.0), (180.0, np.pi)):
+        y = o.init_ray(a, 1000.0, inc, 0.0, 0.0)
+        assert np.all(np.isfinite(y)) and y[1] == 1000.0 and abs(y[2] - th0) < 2e-13 and y[6] == 0.0 and y[7] == 0.0
+        assert abs(o.invariants(a, y)[0] - 1) < 1e-13
+
+
 def test_init_ray_direction_is_parallel_to_observer_axis():
     # flat-space limit (r_obs huge): the Cartesian velocity of every pixel's photon is (sin i, 0, cos i)
     a, inc, robs = 0.0, 35.0, 1e7
