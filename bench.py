@@ -496,7 +496,9 @@ def run_gray(args):
                 "lane_efficiency": rf["lane_efficiency"], "packed_pipe_fraction_measured": mix,
                 "hbm_algorithmic_bytes_per_launch": n * (2 * (32 if args.prec == "f32" else 64) + 10)}
     if args.system == "reduced":
-        roofline["note"] = "system=reduced: no operation tally of its own; see value / ns_per_photon_step"
+        roofline["flops_per_photon_step"] = rf["flops_per_photon_step"]
+        roofline["note"] = ("system=reduced: the oracle's reduced formulation tallies more operations per step than its full one "
+                            "(it evaluates the full right-hand side and discards two equations), so frac can exceed 1; see frac_executed")
     out = {"metric": "photon-steps/s", "value": value, "unit": "photon-steps/s", "n_gpus": world, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": m["ms"] / args.steps, "higher_is_better": True, "scaling": "weak",
            "vs_baseline": None, "dtype": args.prec, "data": "synthetic", "config": workload_config(args, world),
@@ -526,6 +528,11 @@ def run_gray(args):
                                "ns_per_photon_step": 1e9 * dt / ps,
                                "one_core": {"value": ps1 / dt1, "unit": "photon-steps/s", "cores": 1, "ns_per_photon_step": 1e9 * dt1 / ps1,
                                             "sample": f"{m1} photons of the same strided sample, {ps1} photon-steps in {dt1:.1f} s"}}
+        # like for like next to the mixed-precision ratio: the oracle computes in fp64, so the fp64 build is its
+        # counterpart; vs_baseline stays null (BASELINE.md holds no published number for this metric and workload)
+        f64 = [s2["value"] for s2 in secondary if s2["dtype"] == "f64"] if secondary else []
+        out["cpu_baseline"]["gpu_over_oracle"] = {"this_line_%s" % args.prec: value / (ps / dt),
+                                                  "f64_build_same_run": (f64[0] / (ps / dt)) if f64 else None}
     print(json.dumps(out), flush=True)
     if world > 1:
         R.dist.destroy_process_group()

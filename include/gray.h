@@ -139,7 +139,7 @@ GRAY_API int gray_init_rays_polar(gray_state* state, double a, double r_obs, dou
                          int32_t n_R, int32_t n_theta, uint64_t p0, void* cuda_stream);
 
 typedef struct {
-  double h;                  /* step parameter, the paper's Delta ~ 1/32                      */
+  double h;                  /* step parameter, the paper's Delta ~ 1/32; > 0, and <= 0.2 with GRAY_STEP_EQ2 */
   double r_capture_factor;   /* captured when r < factor * r_bh (configs: 1.01); if 0, the paper's    */
   double horizon_delta;      /*   r < r_bh + horizon_delta (delta ~ 1e-6) is used instead       */
   double r_escape_factor;    /* escaped when r > factor * r_obs (configs: 1.01)                       */

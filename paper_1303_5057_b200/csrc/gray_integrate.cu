@@ -146,10 +146,15 @@ integrate_kernel(const __grid_constant__ IntegrateArgs<V> A) {
       if (st != GRAY_LIVE) continue;
       if (s >= A.max_steps) { ++c_live; continue; }
       const typename Vec4T<S>::type xv = A.x[p], kv = A.k[p];
-      S th = xv.z, kh = kv.z;
+      S th = xv.z, kh = kv.z, ph = xv.w;
       int m = 0;
-      if (th > S(1.57079632679489661923)) { th = pi_minus(th); kh = sneg(kh); m = 1; }
-      ys[0][l] = xv.x; ys[1][l] = xv.y - vget(K.rp, 0); ys[2][l] = th; ys[3][l] = xv.w;
+      {
+        // eq. (3) first (a state uploaded by the caller may carry a polar angle outside [0, pi]; one stored by this
+        // library never does), then the fold into [0, pi/2]: the first-stage sine / cosine is fitted on the folded range
+        S unused0 = S(0), unused1 = S(0);
+        remap_theta(th, ph, kh, unused0, unused1, m, true);
+      }
+      ys[0][l] = xv.x; ys[1][l] = xv.y - vget(K.rp, 0); ys[2][l] = th; ys[3][l] = ph;
       ys[4][l] = kv.x; ys[5][l] = kv.y; ys[6][l] = kh; ys[7][l] = kv.w;
 #pragma unroll
       for (int i = 0; i < 8; ++i) cs[i][l] = S(0);
@@ -486,6 +491,11 @@ int gray_integrate(gray_state* state, uint64_t n_photons, uint32_t max_steps, co
   }
   if (params->photons_per_thread < 0 || params->photons_per_thread > 2) { set_error("photons_per_thread must be 0 (default), 1 or 2"); return GRAY_ERR_ARG; }
   if (params->photons_per_thread == 2 && state->prec != GRAY_F32) { set_error("photons_per_thread = 2 (packed FP32 instructions) needs GRAY_F32"); return GRAY_ERR_UNSUPPORTED; }
+  if (params->rule == GRAY_STEP_EQ2 && params->h > 0.2) {
+    // under eq. (2) a step moves theta by at most h; the folded first-stage sine / cosine covers [-0.2, pi/2 + 0.2]
+    set_error("h = %g: GRAY_STEP_EQ2 supports 0 < h <= 0.2 (the paper's Delta ~ 1/32, P:79)", params->h);
+    return GRAY_ERR_DOMAIN;
+  }
   if (!(params->h > 0.0) || !(params->r_escape_factor > 0.0) || params->r_capture_factor < 0.0 ||
       (params->r_capture_factor == 0.0 && !(params->horizon_delta >= 0.0))) {
     set_error("step parameters out of domain (h > 0, r_escape_factor > 0, r_capture_factor >= 0, horizon_delta >= 0)");

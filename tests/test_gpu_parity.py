@@ -639,6 +639,49 @@ def test_edge_cases_empty_single_partial_and_errors():
         g.gray_shadow_edge(br, 16)                                  # random pixels have no image grid
 
 
+@pytest.mark.parametrize("prec,kw", [(g.GRAY_F32, dict()), (g.GRAY_F64, dict()), (g.GRAY_F32, dict(system=g.SYS_REDUCED))])
+def test_uploaded_polar_angle_outside_0_pi_is_remapped_on_load(prec, kw):
+    # a state uploaded by the caller may name its point with theta outside [0, pi]; eq. (3), maps
+    # (-theta, phi + pi, -k^theta) and (2 pi - theta, phi + pi, -k^theta) to the same point as (theta, phi, k^theta).
+    # The kernel applies it when it loads the photon (its first-stage sine / cosine is fitted on the folded range only),
+    # so all three uploads give the same ray: every component but phi bit for bit (phi feeds nothing back and differs
+    # by the rounding of phi + pi - pi).
+    a, inc, W, nx, ny = 0.9, 60.0, 10.0, 40, 30
+    n = nx * ny
+    base = g.PhotonBatch(n, prec)
+    g.gray_init_rays(base, a, wl.R_OBS, inc, W, nx, ny)
+    x0, k0 = base.x.clone(), base.k.clone()
+    g.gray_integrate(base, params=g.StepParams(rule=g.STEP_EQ2, **kw))
+    for variant in ("below 0", "above pi"):
+        b = g.PhotonBatch(n, prec)
+        g.gray_init_rays(b, a, wl.R_OBS, inc, W, nx, ny)
+        b.x[:, 2] = -x0[:, 2] if variant == "below 0" else 2 * np.pi - x0[:, 2]
+        b.x[:, 3] = x0[:, 3] + np.pi
+        b.k[:, 2] = -k0[:, 2]
+        # ("above pi": 2 pi - theta is rounded on upload, so that ray starts one rounding away and is compared to tolerance)
+        g.gray_integrate(b, params=g.StepParams(rule=g.STEP_EQ2, **kw))
+        assert torch.equal(b.status, base.status)
+        if variant == "below 0":
+            for u, v in ((b.x[:, :3], base.x[:, :3]), (b.k, base.k)):
+                assert torch.equal(u.contiguous().view(torch.uint8), v.contiguous().view(torch.uint8)), variant
+            assert torch.equal(b.steps, base.steps)
+        else:
+            ok = (b.status == base.status) & (b.steps == base.steps)
+            assert ok.float().mean() > 0.98
+            err = ((b.x[ok][:, 1:3] - base.x[ok][:, 1:3]).abs() / base.x[ok][:, 1:3].abs().clamp_min(1e-2)).max().item()
+            assert err <= (1e-3 if prec == g.GRAY_F32 else 1e-9), err
+        dphi = torch.remainder((b.x[:, 3] - base.x[:, 3]).double(), 2 * np.pi)           # phi is an angle: compare modulo 2 pi
+        dphi = torch.minimum(dphi, 2 * np.pi - dphi)
+        same = b.steps == base.steps
+        tol_phi = (1e-5 if prec == g.GRAY_F32 else 1e-13) if variant == "below 0" else (1e-3 if prec == g.GRAY_F32 else 1e-9)
+        assert float(dphi[same].max()) <= tol_phi * max(1.0, float(base.x[:, 3].abs().max()))
+    with pytest.raises(g.GrayError, match="0.2"):
+        g.gray_integrate(base, params=g.StepParams(rule=g.STEP_EQ2, h=0.21, **kw))      # beyond the folded range: refused
+    g.gray_integrate(base, params=g.StepParams(rule=g.STEP_EQ2, h=0.2, **kw))           # the largest h accepted
+    if "system" not in kw:
+        g.gray_integrate(base, params=g.StepParams(rule=g.STEP_REL, h=0.5))              # REL range-tests photon by photon
+
+
 def test_integrate_host_matches_device_path():
     # the end-to-end entry point (host buffers, chunked, two streams) gives the device path's bits
     a, inc, W, nx, ny = 0.9, 60.0, 10.0, 100, 77
